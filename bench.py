@@ -1,0 +1,301 @@
+#!/usr/bin/env python3
+"""bench.py -- headline benchmark: real spherical harmonics, lmax = 9, fp64, on the full 128^3 grid
+(BASELINE.json configs[2]), both output layouts.
+
+One "step" = one pass of the whole hot path over the grid for each layout named by the config:
+    sh_real(xyz, n, 9, out_soa, SOA) ; sh_real(xyz, n, 9, out_aos, AOS)        (2 kernel launches)
+`value` counts harmonic values produced per second by the whole job (all ranks), inputs resident in HBM.
+Output buffers (1.68 GB each) are far larger than L2 (126 MB); inputs and outputs rotate between
+replicas so nothing is re-read from L2 between timed iterations.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+N > 1 is launched by torchrun (one rank per GPU); points are independent, so ranks run the same-size
+grid with no data-path collective ("weak" scaling); timing is the max over ranks of CUDA-event time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+LMAX = 9
+K = (LMAX + 1) ** 2
+METRIC = "G harmonic values/s, real SH lmax=9 fp64 (HBM write GB/s in roofline)"
+UNIT = "G values/s"
+WORKLOAD = "configs[2]: real SH lmax=9 fp64, full 128^3 grid over [-6,6]^3 (2,097,152 points), SoA [100][N] + AoS [N][100]"
+BYTES_PER_POINT = 24 + 8 * K  # algorithmic: xyz in + (lmax+1)^2 doubles out
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(kernel_key: str):
+    """Per-launch DRAM bytes of the dominant kernel from the committed ncu summary, or None."""
+    try:
+        return json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))[kernel_key]["dram_bytes_per_launch"]
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    QUERY = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown," \
+            "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(
+                ["nvidia-smi", "-i", str(index), f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits", "-lms", "50"],
+                stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 8:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1]))
+            except ValueError:
+                continue
+            for name, v in zip(names, c[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out = {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
+        return out
+
+
+def grid_points():
+    from paper_2510_05282_b200 import inputs
+
+    return inputs.config3_full_grid()
+
+
+def cpu_baseline(pts, target_seconds=12.0):
+    """The oracle as it stands on this box's host cores, on a bounded prefix-sample of the same workload."""
+    import oracle
+
+    oracle.build()
+    t0 = time.perf_counter()
+    oracle.real(pts[: 1 << 13], LMAX)
+    rate = (1 << 13) / max(time.perf_counter() - t0, 1e-9)  # points/s, calibration
+    m = int(min(len(pts), max(1 << 13, rate * target_seconds)))
+    t0 = time.perf_counter()
+    oracle.real(pts[:m], LMAX)
+    dt = time.perf_counter() - t0
+    return {
+        "value": m * K / dt / 1e9, "unit": UNIT, "cores": oracle.threads_used(), "kind": "oracle",
+        "sample": f"first {m} points of the 128^3 grid, lmax=9 real, long double, one evaluation, {dt:.2f} s",
+    }
+
+
+def run_reference(args):
+    """--impl reference: the oracle is the reference arm for this tier (no upstream code exists)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+
+    oracle.build()
+    pts = grid_points()
+    m = 1 << 15  # bounded sample per step: 32,768 grid points, evaluated once per layout
+    stride = len(pts) // m
+    sample = np.ascontiguousarray(pts[::stride][:m])
+
+    def step():
+        a = oracle.real(sample, LMAX)                      # AoS [m][100]
+        b = np.ascontiguousarray(oracle.real(sample, LMAX).T)  # SoA [100][m]
+        return a, b
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    value = args.steps * 2 * m * K / dt / 1e9
+    cores = oracle.threads_used()
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64 result (oracle computes in x87 long double)", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "sample": f"every {stride}th grid point, {m} points per layout per step"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"{m} strided grid points x 2 layouts per step"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2510_05282_b200 as sh
+
+    sh.load()  # no fallback: fails here if libshb200.so is missing
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the CUDA path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    pts = grid_points()
+    n = len(pts)
+    nrep_in, nrep_out = 4, 2  # 4 x 50 MB inputs > L2; outputs 1.68 GB each
+    xs = [torch.from_numpy(pts).to(dev) for _ in range(nrep_in)]
+    out_soa = [torch.empty((K, n), dtype=torch.float64, device=dev) for _ in range(nrep_out)]
+    out_aos = [torch.empty((n, K), dtype=torch.float64, device=dev) for _ in range(nrep_out)]
+    stream = torch.cuda.current_stream(dev)
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def step(it, marks=None):
+        x = xs[it % nrep_in]
+        if marks is not None:
+            e0, e1, e2 = ev(), ev(), ev()
+            e0.record(stream)
+        sh.sh_real(x, LMAX, out=out_soa[it % nrep_out], layout="soa")
+        if marks is not None:
+            e1.record(stream)
+        sh.sh_real(x, LMAX, out=out_aos[it % nrep_out], layout="aos")
+        if marks is not None:
+            e2.record(stream)
+            marks.append((e0, e1, e2))
+
+    for it in range(max(args.warmup, 3)):
+        step(it)
+    torch.cuda.synchronize()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    launches0 = sh.kernel_launch_count()
+    marks = []
+    start, end = ev(), ev()
+    torch.cuda.synchronize()
+    start.record(stream)
+    for it in range(args.steps):
+        step(it, marks)
+    end.record(stream)
+    torch.cuda.synchronize()
+    barrier()
+    launches = sh.kernel_launch_count() - launches0
+    clocks = sampler.stop() if sampler else None
+    ms = start.elapsed_time(end)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    t_soa = sum(a.elapsed_time(b) for a, b, _ in marks) / len(marks)
+    t_aos = sum(b.elapsed_time(c) for _, b, c in marks) / len(marks)
+
+    # end to end through the C ABI with HOST buffers (pinned): H2D of xyz and D2H of every result inside the timed region
+    e2e_steps = max(1, min(args.steps, 3))
+    hx = torch.from_numpy(pts).pin_memory()
+    h_soa = torch.empty((K, n), dtype=torch.float64).pin_memory()
+    h_aos = torch.empty((n, K), dtype=torch.float64).pin_memory()
+
+    def e2e_step():
+        sh.host_call("real", hx, LMAX, out=h_soa, layout="soa")
+        sh.host_call("real", hx, LMAX, out=h_aos, layout="aos")
+
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    # spot-check the end-to-end result against the device-resident result
+    assert torch.equal(h_aos[:1000], out_aos[(args.steps - 1) % nrep_out][:1000].cpu())
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        dom = ("sh_real lmax=9 SoA", t_soa, "soa") if t_soa >= t_aos else ("sh_real lmax=9 AoS", t_aos, "aos")
+        achieved = BYTES_PER_POINT * n / (dom[1] * 1e-3) / 1e9
+        values_per_step = 2 * n * K
+        line = {
+            "metric": METRIC, "value": world * args.steps * values_per_step / (ms * 1e-3) / 1e9, "unit": UNIT,
+            "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "points_per_gpu": n, "lmax": LMAX, "calls_per_step": ["sh_real SOA", "sh_real AOS"],
+                       "l2": "outputs (1.68 GB per call) and rotating input replicas (4 x 50 MB) exceed the 126 MB L2"},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "kernels": {
+                "sh_real_soa": {"ms": t_soa, "write_GBps": 8 * K * n / (t_soa * 1e-3) / 1e9, "G_values_per_s": n * K / (t_soa * 1e-3) / 1e9},
+                "sh_real_aos": {"ms": t_aos, "write_GBps": 8 * K * n / (t_aos * 1e-3) / 1e9, "G_values_per_s": n * K / (t_aos * 1e-3) / 1e9},
+            },
+            "roofline": {
+                "bound": "hbm", "kernel": dom[0], "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": BYTES_PER_POINT * n, "avg_launch_ms": dom[1],
+                "traffic": ncu_traffic(dom[2]),
+            },
+            "e2e": {"value": world * e2e_steps * values_per_step / e2e_s / 1e9, "unit": UNIT,
+                    "h2d_bytes_per_step": 2 * n * 24, "d2h_bytes_per_step": 2 * n * K * 8, "steps": e2e_steps,
+                    "api": "sh_real_host (pinned host buffers)"},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(pts)
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

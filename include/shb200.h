@@ -1,0 +1,112 @@
+/*
+ * shb200.h -- C ABI of libshb200: batched real, complex and spin-1/2 spinor spherical harmonics for
+ * all l <= lmax <= 9 at Cartesian points, on one NVIDIA B200 (sm_100a).
+ *
+ * The operation is the one stated in arxiv 2510.05282 ("SHarmonic"); citations are to
+ * /root/reference/PAPER.md lines (P:n) and to this repository's DESIGN.md:
+ *   - Y_l^m, Condon-Shortley phase included:        Eq. 5
+ *   - real harmonics R_l^m:                          Eq. 6
+ *   - spinor harmonics, spin 1/2, j = l +- 1/2:      Eq. 7
+ *   - Cartesian front end, the value does not depend on |r|;
+ *     at r = 0 every harmonic is 0 except l = 0:
+ *   - evaluated as explicit factorized polynomials in x/r, y/r, z/r: Eq. 8, Eq. 16, App. B/C
+ *
+ * Conventions (the paper's API is per point and per (l, m) and fixes no batch layout):
+ *   K = (lmax+1)^2.  Point i, harmonic index k = l(l+1)+m, m = -l..l.
+ *   real     element = 1 double           count per point = K
+ *   complex  element = (re, im)           count per point = K      (2K doubles)
+ *   spinor   element = (up.re, up.im, down.re, down.im)            count per point = 2K (8K doubles)
+ *            s = 2 l^2 + (j = l-1/2 ? m_j + j : 2l + m_j + j): l ascending; the j = l-1/2 block (2l entries,
+ *            absent for l = 0) then the j = l+1/2 block (2l+2 entries); m_j ascending.
+ *   SH_LAYOUT_AOS: out[i * count + e]   ([N][count] elements)
+ *   SH_LAYOUT_SOA: out[e * n + i]       ([count][N] elements; an element stays contiguous)
+ *
+ * Pointers: every `xyz` / `out` of the sh_real / sh_complex / sh_spinor / sh_real_f32 calls is a DEVICE
+ * pointer (global memory of the current CUDA device); `xyz` is AoS [n][3].  The *_host calls take HOST
+ * pointers.  The caller owns all buffers; the library allocates nothing on the device calls, keeps no
+ * state between calls and is re-entrant.  Device calls are asynchronous: they enqueue kernels on
+ * `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream) and return without
+ * synchronizing.  `out` must be aligned to its element type (8 B for sh_real, 4 B for sh_real_f32); 16-byte
+ * aligned `out` (and, for SoA, even n) enables the vectorised / bulk-copy store paths, anything else falls
+ * back to a scalar store path with identical results.  `xyz` and `out` must not overlap.
+ *
+ * Domain: any finite coordinates, including subnormal and huge ones (inputs are pre-scaled by a power
+ * of two before r^2 is formed); r = 0 exactly (no epsilon) selects the P:60 convention.  NaN or Inf
+ * coordinates give NaN outputs for that point (not an error).
+ *
+ * Errors: every call returns SH_OK (0) or a negative SH_ERR_* code; nothing is thrown and nothing is
+ * written on error.  n == 0 is a successful no-op (pointers may then be NULL).
+ */
+#ifndef SHB200_H
+#define SHB200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    SH_LAYOUT_AOS = 0, /* out[i*count + e] */
+    SH_LAYOUT_SOA = 1  /* out[e*n + i]     */
+};
+
+/* Optional store-path request, OR-ed into `layout` (bits 8-15).  SH_STORE_AUTO picks the fastest path the
+ * alignment allows.  A request the alignment does not allow returns SH_ERR_ALIGNMENT.  Results are identical
+ * on every path (same arithmetic, different store mechanism). */
+enum {
+    SH_STORE_AUTO   = 0 << 8,
+    SH_STORE_DIRECT = 1 << 8, /* per-thread st.global.cs; SoA: coalesced planes; AoS: smem transpose + coalesced stores */
+    SH_STORE_BULK   = 2 << 8  /* AoS only: per-point rows staged in shared memory, written by TMA bulk copies (cp.async.bulk) */
+};
+
+enum {
+    SH_OK = 0,
+    SH_ERR_NULL = -1,      /* xyz or out is NULL with n > 0 */
+    SH_ERR_COUNT = -2,     /* n < 0 */
+    SH_ERR_LMAX = -3,      /* lmax outside [0, 9] */
+    SH_ERR_LAYOUT = -4,    /* unknown layout or store-path bits */
+    SH_ERR_ALIGNMENT = -5, /* out not aligned to its element type, or requested store path not possible */
+    SH_ERR_CUDA = -6       /* CUDA launch / copy error; text via sh_last_cuda_error() */
+};
+
+/* Real harmonics R_l^m (Eq. 6), fp64.  out: K doubles per point. */
+int sh_real(const double* xyz, int64_t n, int lmax, double* out, int layout, void* stream);
+/* Complex harmonics Y_l^m (Eq. 5), fp64.  out: K (re, im) pairs per point. */
+int sh_complex(const double* xyz, int64_t n, int lmax, double* out, int layout, void* stream);
+/* Spinor harmonics (Eq. 7), fp64.  out: 2K elements of 4 doubles per point. */
+int sh_spinor(const double* xyz, int64_t n, int lmax, double* out, int layout, void* stream);
+/* fp32 variant of sh_real: fp32 in, fp32 out; the normalization runs in fp64, the polynomials in fp32. */
+int sh_real_f32(const float* xyz, int64_t n, int lmax, float* out, int layout, void* stream);
+
+/* Host-buffer entry points: same results, `xyz` and `out` are HOST pointers (pinned memory gives full
+ * PCIe speed; pageable memory works).  The call copies chunks host->device, runs the kernels and copies
+ * device->host on internal streams with double buffering, and returns after `out` is complete.  It
+ * allocates and frees its own device staging buffers (at most ~1 GiB). */
+int sh_real_host(const double* xyz, int64_t n, int lmax, double* out, int layout);
+int sh_complex_host(const double* xyz, int64_t n, int lmax, double* out, int layout);
+int sh_spinor_host(const double* xyz, int64_t n, int lmax, double* out, int layout);
+int sh_real_f32_host(const float* xyz, int64_t n, int lmax, float* out, int layout);
+
+/* Scalars (doubles for the fp64 calls, floats for sh_real_f32) written per point; -1 if lmax is out of range. */
+int64_t sh_real_count(int lmax);    /* K   */
+int64_t sh_complex_count(int lmax); /* 2K  */
+int64_t sh_spinor_count(int lmax);  /* 8K  */
+
+/* Element index of (l, m) in the real / complex outputs: l(l+1)+m; -1 if out of range. */
+int sh_index_real(int l, int m);
+/* Element index of (l, j, m_j) in the spinor output; half-integers are passed doubled (twoj = 2j, twomj = 2m_j);
+ * -1 if the triple is not a valid spin-1/2 state with l <= 9. */
+int sh_index_spinor(int l, int twoj, int twomj);
+
+/* Static text for an SH_ERR_* code. */
+const char* sh_strerror(int code);
+/* Text of the last CUDA error seen by this thread's calls ("" if none). */
+const char* sh_last_cuda_error(void);
+/* Number of kernels this library has launched in this process (for launch accounting in benchmarks). */
+int64_t sh_kernel_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SHB200_H */

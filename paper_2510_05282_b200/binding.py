@@ -1,0 +1,160 @@
+"""Thin ctypes binding over libshb200.so (include/shb200.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels; PyTorch is used for device memory and streams.
+There is no CPU fallback: if the shared library is missing or a call fails, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+SH_LAYOUT_AOS = 0
+SH_LAYOUT_SOA = 1
+SH_STORE_AUTO = 0 << 8
+SH_STORE_DIRECT = 1 << 8
+SH_STORE_BULK = 2 << 8
+
+_LAYOUTS = {"aos": SH_LAYOUT_AOS, "soa": SH_LAYOUT_SOA, SH_LAYOUT_AOS: SH_LAYOUT_AOS, SH_LAYOUT_SOA: SH_LAYOUT_SOA}
+_STORES = {"auto": SH_STORE_AUTO, "direct": SH_STORE_DIRECT, "bulk": SH_STORE_BULK}
+
+LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libshb200.so")
+_lib = None
+
+
+class ShError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        lib = load()
+        msg = lib.sh_strerror(code).decode()
+        if code == -6:
+            msg += ": " + lib.sh_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg} (code {code})")
+        self.code = code
+
+
+def load() -> ctypes.CDLL:
+    """Load libshb200.so; raises if it has not been built (python -m paper_2510_05282_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(
+                f"{LIB_PATH} not found: build it with `python -m paper_2510_05282_b200.build` (no CPU fallback exists)"
+            )
+        lib = ctypes.CDLL(LIB_PATH)
+        vp, i64, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
+        for name in ("sh_real", "sh_complex", "sh_spinor", "sh_real_f32"):
+            f = getattr(lib, name)
+            f.argtypes = [vp, i64, ci, vp, ci, vp]
+            f.restype = ci
+            h = getattr(lib, name + "_host")
+            h.argtypes = [vp, i64, ci, vp, ci]
+            h.restype = ci
+        for name in ("sh_real_count", "sh_complex_count", "sh_spinor_count"):
+            getattr(lib, name).argtypes = [ci]
+            getattr(lib, name).restype = i64
+        lib.sh_index_real.argtypes = [ci, ci]
+        lib.sh_index_real.restype = ci
+        lib.sh_index_spinor.argtypes = [ci, ci, ci]
+        lib.sh_index_spinor.restype = ci
+        lib.sh_strerror.argtypes = [ci]
+        lib.sh_strerror.restype = ctypes.c_char_p
+        lib.sh_last_cuda_error.restype = ctypes.c_char_p
+        lib.sh_kernel_launch_count.restype = i64
+        _lib = lib
+    return _lib
+
+
+def layout_bits(layout, store="auto") -> int:
+    return _LAYOUTS[layout] | _STORES[store]
+
+
+def count(kind: str, lmax: int) -> int:
+    """Scalars written per point."""
+    return int(getattr(load(), f"sh_{'real' if kind == 'real_f32' else kind}_count")(lmax))
+
+
+def index_real(l: int, m: int) -> int:
+    return load().sh_index_real(l, m)
+
+
+def index_spinor(l: int, twoj: int, twomj: int) -> int:
+    return load().sh_index_spinor(l, twoj, twomj)
+
+
+def kernel_launch_count() -> int:
+    return int(load().sh_kernel_launch_count())
+
+
+def out_shape(kind: str, n: int, lmax: int, layout) -> tuple:
+    """Shape of `out` in scalars: AoS [n][K*es], SoA [K][n*es] flattened per element as [K][n][es]."""
+    k = (lmax + 1) ** 2
+    es = {"real": 1, "real_f32": 1, "complex": 2, "spinor": 4}[kind]
+    ne = 2 * k if kind == "spinor" else k
+    if _LAYOUTS[layout] == SH_LAYOUT_AOS:
+        return (n, ne, es) if es > 1 else (n, ne)
+    return (ne, n, es) if es > 1 else (ne, n)
+
+
+def _device_call(kind: str, xyz, lmax: int, out, layout, store, stream):
+    import torch
+
+    fn = getattr(load(), "sh_" + kind)
+    want = torch.float32 if kind == "real_f32" else torch.float64
+    if not (xyz.is_cuda and xyz.dtype == want and xyz.is_contiguous() and xyz.dim() == 2 and xyz.shape[1] == 3):
+        raise ValueError("xyz must be a contiguous CUDA tensor [n][3] of " + str(want))
+    n = xyz.shape[0]
+    shape = out_shape(kind, n, lmax, layout)
+    if out is None:
+        out = torch.empty(shape, dtype=want, device=xyz.device)
+    elif not (out.is_cuda and out.dtype == want and out.is_contiguous() and out.numel() == int(np.prod(shape))):
+        raise ValueError(f"out must be a contiguous CUDA tensor of {want} with {int(np.prod(shape))} elements")
+    s = torch.cuda.current_stream(xyz.device).cuda_stream if stream is None else int(stream)
+    with torch.cuda.device(xyz.device):
+        rc = fn(xyz.data_ptr(), n, int(lmax), out.data_ptr(), layout_bits(layout, store), s)
+    if rc != 0:
+        raise ShError(rc, "sh_" + kind)
+    return out
+
+
+def sh_real(xyz, lmax, out=None, layout="soa", store="auto", stream=None):
+    """R_l^m (Eq. 6) for l <= lmax at CUDA tensor xyz [n][3] float64 -> AoS [n][K] or SoA [K][n]."""
+    return _device_call("real", xyz, lmax, out, layout, store, stream)
+
+
+def sh_complex(xyz, lmax, out=None, layout="soa", store="auto", stream=None):
+    """Y_l^m (Eq. 5) -> AoS [n][K][2] or SoA [K][n][2] float64 (re, im)."""
+    return _device_call("complex", xyz, lmax, out, layout, store, stream)
+
+
+def sh_spinor(xyz, lmax, out=None, layout="soa", store="auto", stream=None):
+    """Spinor harmonics (Eq. 7) -> AoS [n][2K][4] or SoA [2K][n][4] float64 (up.re, up.im, down.re, down.im)."""
+    return _device_call("spinor", xyz, lmax, out, layout, store, stream)
+
+
+def sh_real_f32(xyz, lmax, out=None, layout="soa", store="auto", stream=None):
+    """fp32 variant of sh_real (float32 in, float32 out)."""
+    return _device_call("real_f32", xyz, lmax, out, layout, store, stream)
+
+
+def host_call(kind: str, xyz: "np.ndarray | object", lmax: int, out=None, layout="soa"):
+    """sh_*_host: HOST buffers in and out (numpy arrays or CPU torch tensors, ideally pinned)."""
+    fn = getattr(load(), f"sh_{kind}_host")
+    dt = np.float32 if kind == "real_f32" else np.float64
+
+    def ptr_n(a):
+        if hasattr(a, "data_ptr"):
+            return a.data_ptr(), a
+        a = np.ascontiguousarray(a, dtype=dt)
+        return a.ctypes.data, a
+
+    xp, xk = ptr_n(xyz)
+    n = xk.shape[0]
+    shape = out_shape(kind, n, lmax, layout)
+    if out is None:
+        out = np.empty(shape, dtype=dt)
+    op, ok = ptr_n(out)
+    rc = fn(xp, n, int(lmax), op, _LAYOUTS[layout])
+    if rc != 0:
+        raise ShError(rc, f"sh_{kind}_host")
+    return ok

@@ -1,0 +1,633 @@
+// shb200.cu -- sm_100a kernels + C ABI (include/shb200.h) for batched spherical harmonics, l <= 9.
+//
+// Hot path per point (P:n = /root/reference/PAPER.md line n):
+//   a1 load xyz (AoS [N][3])
+//   a2 normalize: x, y, z <- (x, y, z)/r, r = 0 flag          P:58-69, Eq. 8
+//   a3 azimuthal factors C_m, S_m (root-pair products)        Eq. 16, App. B
+//   a4 polar factors Qhat_l^m(z) (root-pair products)         Eq. 14-15
+//   a5 combine -> R_l^m, r = 0 convention                     Eq. 6
+//   a6 complex Y_l^m                                          Eq. 5, 9, 10 P:42
+//   a7 spinor harmonics                                       Eq. 7
+//   a8 store: SoA planes by coalesced streaming stores; AoS rows staged in shared memory and written
+//      by TMA bulk copies (cp.async.bulk.global.shared::cta) or by coalesced stores.
+// a3/a4 building blocks and all constants come from the build-time generator (sh_generated.cuh).
+//
+// One thread evaluates one point; all (lmax+1)^2 values of a point are produced in ascending k by
+// straight-line code, so the store sinks below see compile-time offsets only.
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cfloat>
+#include <cstdint>
+#include <cstring>
+#include <type_traits>
+
+#include "../../include/shb200.h"
+#include "sh_generated.cuh"
+
+namespace {
+
+constexpr int KIND_REAL = 0, KIND_COMPLEX = 1, KIND_SPINOR = 2;
+constexpr int MODE_PLAIN = 0, MODE_ROWBULK = 1;
+
+// ------------------------------------------------------------------------------------------------
+// compile-time loop
+template <int B, int E, class F>
+__device__ __forceinline__ void static_for(F&& f) {
+    if constexpr (B < E) {
+        f(std::integral_constant<int, B>{});
+        static_for<B + 1, E>(f);
+    }
+}
+
+// scalars (T) per element, elements per point
+__host__ __device__ constexpr int elem_scalars(int kind) { return kind == KIND_REAL ? 1 : kind == KIND_COMPLEX ? 2 : 4; }
+__host__ __device__ constexpr int elems_per_point(int kind, int lmax) {
+    return (kind == KIND_SPINOR ? 2 : 1) * (lmax + 1) * (lmax + 1);
+}
+__host__ __device__ constexpr int scalars_per_point(int kind, int lmax) { return elem_scalars(kind) * elems_per_point(kind, lmax); }
+// scalars of a point's row that precede the l-block
+__host__ __device__ constexpr int cum_scalars(int kind, int l) { return (kind == KIND_REAL ? 1 : kind == KIND_COMPLEX ? 2 : 8) * l * l; }
+
+// ------------------------------------------------------------------------------------------------
+// a2: normalization.  fp64 always (also for the fp32 variant).
+struct UnitVec {
+    double x, y, z;
+    bool origin;
+};
+
+__device__ __forceinline__ UnitVec normalize(double x, double y, double z) {
+    // keep r^2 finite and normal over the whole fp64 range: scale by an exact power of two when needed
+    const double s = fmax(fmax(fabs(x), fabs(y)), fabs(z));
+    if (s < 0x1p-500) {
+        x *= 0x1p600; y *= 0x1p600; z *= 0x1p600;
+    } else if (s > 0x1p500) {
+        x *= 0x1p-600; y *= 0x1p-600; z *= 0x1p-600;
+    }
+    const double r2 = x * x + y * y + z * z;
+    UnitVec u;
+    u.origin = (r2 == 0.0);
+    double inv = 1.0 / sqrt(r2);                          // IEEE sqrt and divide
+    if (u.origin) inv = 0.0;                              // r = 0: (0, 0, 0), handled by the evaluators
+    if (!(r2 <= DBL_MAX)) inv = __longlong_as_double(0x7ff8000000000000LL);  // NaN / Inf input -> NaN outputs
+    u.x = x * inv; u.y = y * inv; u.z = z * inv;
+    return u;
+}
+
+template <typename TI>
+__device__ __forceinline__ UnitVec load_unit(const TI* __restrict__ xyz, int64_t i) {
+    const TI* p = xyz + 3 * i;
+    return normalize((double)__ldg(p), (double)__ldg(p + 1), (double)__ldg(p + 2));
+}
+
+// ------------------------------------------------------------------------------------------------
+// a3-a7: evaluators.  Sink interface: put1<K>(v) real element K; put2<K>(re, im) complex element K;
+// put4<S>(ur, ui, dr, di) spinor element S; end_l<L>() after the last element of block l.
+template <int LMAX, typename T>
+struct Azim {
+    T C[LMAX + 1], S[LMAX + 1];
+    __device__ __forceinline__ Azim(T x, T y) {
+        static_for<0, LMAX + 1>([&](auto mc) {
+            constexpr int M = decltype(mc)::value;
+            shgen::Azimuthal<M, T>::eval(x, y, C[M], S[M]);
+        });
+    }
+};
+
+template <int LMAX, typename T, class Sink>
+__device__ __forceinline__ void eval_real(T x, T y, T z, bool origin, Sink& sink) {
+    const Azim<LMAX, T> az(x, y);
+    static_for<0, LMAX + 1>([&](auto lc) {
+        constexpr int L = decltype(lc)::value;
+        T q[L + 1];
+        static_for<0, L + 1>([&](auto mc) {
+            constexpr int M = decltype(mc)::value;
+            constexpr double A = shgen::A_REAL[L][M];
+            q[M] = T(A) * shgen::Polar<L, M, T>::eval(z);
+        });
+        // r = 0: x = y = z = 0 zeroes everything except the even-l, m = 0 polynomials (P_l(0) != 0)
+        if constexpr (L > 0 && L % 2 == 0) { if (origin) q[0] = T(0); }
+        static_for<0, L>([&](auto jc) {
+            constexpr int M = L - decltype(jc)::value;
+            sink.template put1<L * (L + 1) - M>(q[M] * az.S[M]);
+        });
+        sink.template put1<L * (L + 1)>(q[0]);
+        static_for<1, L + 1>([&](auto mc) {
+            constexpr int M = decltype(mc)::value;
+            sink.template put1<L * (L + 1) + M>(q[M] * az.C[M]);
+        });
+        sink.template end_l<L>();
+    });
+}
+
+// a[M] + i b[M] = B_lm Qhat_lm (C_M + i S_M);  Y_l^{-M} = (a, -b),  Y_l^{+M} = (-1)^M (a, b)
+template <int L, int LMAX, typename T>
+__device__ __forceinline__ void complex_block(const Azim<LMAX, T>& az, T z, bool origin, T (&a)[L + 1], T (&b)[L + 1]) {
+    static_for<0, L + 1>([&](auto mc) {
+        constexpr int M = decltype(mc)::value;
+        constexpr double B = shgen::B_CPLX[L][M];
+        const T u = T(B) * shgen::Polar<L, M, T>::eval(z);
+        a[M] = u * az.C[M];
+        b[M] = u * az.S[M];
+    });
+    if constexpr (L > 0 && L % 2 == 0) { if (origin) a[0] = T(0); }
+}
+
+template <int LMAX, typename T, class Sink>
+__device__ __forceinline__ void eval_complex(T x, T y, T z, bool origin, Sink& sink) {
+    const Azim<LMAX, T> az(x, y);
+    static_for<0, LMAX + 1>([&](auto lc) {
+        constexpr int L = decltype(lc)::value;
+        T a[L + 1], b[L + 1];
+        complex_block<L>(az, z, origin, a, b);
+        static_for<0, L>([&](auto jc) {
+            constexpr int M = L - decltype(jc)::value;
+            sink.template put2<L * (L + 1) - M>(a[M], -b[M]);
+        });
+        sink.template put2<L * (L + 1)>(a[0], T(0));
+        static_for<1, L + 1>([&](auto mc) {
+            constexpr int M = decltype(mc)::value;
+            if constexpr (M % 2) sink.template put2<L * (L + 1) + M>(-a[M], -b[M]);
+            else sink.template put2<L * (L + 1) + M>(a[M], b[M]);
+        });
+        sink.template end_l<L>();
+    });
+}
+
+// component c * Y_l^m from the block's (a, b); c and the signs fold into one compile-time constant
+template <int L, int M_SIGNED, typename T>
+__device__ __forceinline__ void scaled_y(double c, const T (&a)[L + 1], const T (&b)[L + 1], T& re, T& im) {
+    constexpr int M = M_SIGNED < 0 ? -M_SIGNED : M_SIGNED;
+    if constexpr (M > L) {
+        re = T(0); im = T(0);
+    } else if constexpr (M_SIGNED < 0) {
+        re = T(c) * a[M]; im = T(-c) * b[M];
+    } else if constexpr (M_SIGNED == 0) {
+        re = T(c) * a[0]; im = T(0);
+    } else {
+        const double s = (M % 2) ? -c : c;
+        re = T(s) * a[M]; im = T(s) * b[M];
+    }
+}
+
+template <int LMAX, typename T, class Sink>
+__device__ __forceinline__ void eval_spinor(T x, T y, T z, bool origin, Sink& sink) {
+    const Azim<LMAX, T> az(x, y);
+    static_for<0, LMAX + 1>([&](auto lc) {
+        constexpr int L = decltype(lc)::value;
+        T a[L + 1], b[L + 1];
+        complex_block<L>(az, z, origin, a, b);
+        static_for<2 * L * L, 2 * (L + 1) * (L + 1)>([&](auto sc) {
+            constexpr int S = decltype(sc)::value;
+            constexpr shgen::SpinorEntry e = shgen::SPINOR[S];
+            static_assert(e.l == L, "spinor table order");
+            T ur, ui, dr, di;
+            scaled_y<L, e.m_up>(e.cu, a, b, ur, ui);
+            scaled_y<L, e.m_dn>(e.cd, a, b, dr, di);
+            sink.template put4<S>(ur, ui, dr, di);
+        });
+        sink.template end_l<L>();
+    });
+}
+
+template <int KIND, int LMAX, typename T, class Sink>
+__device__ __forceinline__ void evaluate(const UnitVec& u, Sink& sink) {
+    const T x = (T)u.x, y = (T)u.y, z = (T)u.z;   // fp32 variant: rounded once, after the fp64 normalization
+    if constexpr (KIND == KIND_REAL) eval_real<LMAX, T>(x, y, z, u.origin, sink);
+    else if constexpr (KIND == KIND_COMPLEX) eval_complex<LMAX, T>(x, y, z, u.origin, sink);
+    else eval_spinor<LMAX, T>(x, y, z, u.origin, sink);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a8, SoA: element e of point i lives at out[(e*n + i) * ES .. +ES).  A warp writes 32*ES contiguous scalars
+// per element; streaming (evict-first) stores since nothing is re-read.  VEC = widest store in bytes the
+// alignment of `out` allows.
+template <typename T, int VEC>
+struct SoASink {
+    T* p;             // out + i*ES
+    int64_t stride;   // n*ES scalars between consecutive elements
+    template <int K> __device__ __forceinline__ void put1(T v) { __stcs(p + K * stride, v); }
+    template <int K> __device__ __forceinline__ void put2(T re, T im) {
+        T* q = p + K * stride;
+        if constexpr (VEC >= 16 && sizeof(T) == 8) {
+            __stcs(reinterpret_cast<double2*>(q), make_double2(re, im));
+        } else { __stcs(q, re); __stcs(q + 1, im); }
+    }
+    template <int S> __device__ __forceinline__ void put4(T a, T b, T c, T d) {
+        T* q = p + S * stride;
+        if constexpr (VEC >= 32 && sizeof(T) == 8) {
+            asm volatile("st.global.cs.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(q), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+        } else if constexpr (VEC >= 16 && sizeof(T) == 8) {
+            __stcs(reinterpret_cast<double2*>(q), make_double2(a, b));
+            __stcs(reinterpret_cast<double2*>(q) + 1, make_double2(c, d));
+        } else { __stcs(q, a); __stcs(q + 1, b); __stcs(q + 2, c); __stcs(q + 3, d); }
+    }
+    template <int L> __device__ __forceinline__ void end_l() {}
+};
+
+template <int KIND, int LMAX, typename T, typename TI, int VEC>
+__global__ void __launch_bounds__(256) sh_soa_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out) {
+    const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (i >= n) return;
+    const UnitVec u = load_unit(xyz, i);
+    constexpr int ES = elem_scalars(KIND);
+    SoASink<T, VEC> sink{out + i * ES, n * ES};
+    evaluate<KIND, LMAX, T>(u, sink);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a8, AoS: a point's row of SP = scalars_per_point scalars is contiguous in `out`.  Each lane stages its row
+// (or a segment of whole l-blocks of it, at most CAP scalars) in its own shared-memory row, then
+//   MODE_ROWBULK: the lane issues ONE TMA bulk copy (cp.async.bulk.global.shared::cta) for its segment;
+//                 needs 16-byte aligned global segments.  No warp-level synchronization at all.
+//   MODE_PLAIN:   the warp copies the staged tile out with coalesced streaming stores (any alignment).
+template <int KIND, int LMAX, int TSIZE, int CAP, int MODE>
+struct Segments {
+    static constexpr int SP = scalars_per_point(KIND, LMAX);
+    // a cut before block l is allowed where the row offset keeps the copy granularity (16 B for bulk)
+    static constexpr bool cut_ok(int l) { return l == LMAX + 1 || MODE == MODE_PLAIN || (cum_scalars(KIND, l) * TSIZE) % 16 == 0; }
+    // greedy: the segment starting at block s ends before block seg_end(s)
+    static constexpr int seg_end(int s) {
+        int best = -1;
+        for (int c = s + 1; c <= LMAX + 1; ++c)
+            if (cut_ok(c) && cum_scalars(KIND, c) - cum_scalars(KIND, s) <= CAP) best = c;
+        return best;
+    }
+    static constexpr int first_l(int l) {
+        int s = 0;
+        while (seg_end(s) <= l) s = seg_end(s);
+        return s;
+    }
+    static constexpr bool valid() {
+        for (int s = 0; s <= LMAX;) {
+            int e = seg_end(s);
+            if (e < 0) return false;
+            s = e;
+        }
+        return true;
+    }
+    static constexpr int max_len() {
+        int m = 0;
+        for (int s = 0; s <= LMAX; s = seg_end(s)) {
+            int len = cum_scalars(KIND, seg_end(s)) - cum_scalars(KIND, s);
+            if (len > m) m = len;
+        }
+        return m;
+    }
+    // row pitch in scalars: conflict-free staging stores.  bulk: 16-byte stores, odd number of 16-byte chunks;
+    // plain: scalar stores, odd number of 8-byte (fp64) / 4-byte (fp32) words.
+    static constexpr int pitch() {
+        if (MODE == MODE_ROWBULK) {
+            int chunks = (max_len() * TSIZE + 15) / 16;
+            return (chunks | 1) * 16 / TSIZE;
+        }
+        return max_len() | 1;
+    }
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+template <int KIND, int LMAX, typename T, int CAP, int MODE>
+struct RowSink {
+    using Seg = Segments<KIND, LMAX, sizeof(T), CAP, MODE>;
+    static constexpr int SP = Seg::SP;
+    static constexpr int PITCH = Seg::pitch();
+    static constexpr int VPC = 16 / sizeof(T);   // scalars per 16-byte chunk
+
+    T* row;          // this lane's staging row (shared memory)
+    T* tile;         // the warp's staging tile (32 rows)
+    T* gout;         // global `out`
+    int64_t i;       // this lane's point
+    int64_t base;    // first point of the warp's tile
+    int rows;        // valid rows of the tile (plain mode)
+    int lane;
+    T hold[VPC > 1 ? VPC - 1 : 1];
+
+    // scalar offset of row scalar J inside the staging row
+    template <int J, int L> static constexpr int off() { return J - cum_scalars(KIND, Seg::first_l(L)); }
+    template <int K> static constexpr int l_of_real() { int l = 0; while ((l + 1) * (l + 1) <= K) ++l; return l; }
+    template <int S> static constexpr int l_of_spinor() { int l = 0; while (2 * (l + 1) * (l + 1) <= S) ++l; return l; }
+
+    __device__ __forceinline__ void st16(T* dst, T a, T b) { *reinterpret_cast<double2*>(dst) = make_double2(a, b); }
+
+    template <int K> __device__ __forceinline__ void put1(T v) {
+        constexpr int O = off<K, l_of_real<K>()>();
+        if constexpr (MODE == MODE_PLAIN) {
+            row[O] = v;
+        } else if constexpr (sizeof(T) == 8) {
+            if constexpr (K % 2 == 0) hold[0] = v;
+            else st16(row + O - 1, hold[0], v);
+        } else {
+            if constexpr (K % 4 != 3) hold[K % 4] = v;
+            else *reinterpret_cast<float4*>(row + O - 3) = make_float4(hold[0], hold[1], hold[2], v);
+        }
+    }
+    template <int K> __device__ __forceinline__ void put2(T re, T im) {
+        constexpr int O = off<2 * K, l_of_real<K>()>();
+        if constexpr (MODE == MODE_PLAIN) { row[O] = re; row[O + 1] = im; }
+        else st16(row + O, re, im);
+    }
+    template <int S> __device__ __forceinline__ void put4(T a, T b, T c, T d) {
+        constexpr int O = off<4 * S, l_of_spinor<S>()>();
+        if constexpr (MODE == MODE_PLAIN) { row[O] = a; row[O + 1] = b; row[O + 2] = c; row[O + 3] = d; }
+        else { st16(row + O, a, b); st16(row + O + 2, c, d); }
+    }
+
+    __device__ __forceinline__ void wait_reads() {
+        if constexpr (MODE == MODE_ROWBULK) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    }
+
+    template <int L> __device__ __forceinline__ void end_l() {
+        constexpr int S0 = Seg::first_l(L);
+        if constexpr (Seg::seg_end(S0) == L + 1) {
+            constexpr int BEGIN = cum_scalars(KIND, S0);
+            constexpr int LEN = cum_scalars(KIND, L + 1) - BEGIN;
+            if constexpr (MODE == MODE_ROWBULK) {
+                static_assert((LEN * sizeof(T)) % 16 == 0 && (BEGIN * sizeof(T)) % 16 == 0, "bulk granularity");
+                // generic-proxy staging stores -> visible to the async proxy, then one bulk copy for this row segment
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gout + i * SP + BEGIN),
+                             "r"(smem_u32(row)), "r"(LEN * (int)sizeof(T))
+                             : "memory");
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                if constexpr (L < LMAX) wait_reads();   // the row is reused by the next segment
+            } else {
+                __syncwarp();
+                if constexpr (LEN == SP) {
+                    // whole rows staged: the tile is one contiguous span of rows*SP scalars in `out`
+                    T* g = gout + base * SP;
+                    const int total = rows * SP;
+                    int r = 0, c = lane;
+                    while (c >= SP) { c -= SP; ++r; }
+                    for (int e = lane; e < total; e += 32) {
+                        __stcs(g + e, tile[r * PITCH + c]);
+                        c += 32;
+                        while (c >= SP) { c -= SP; ++r; }
+                    }
+                } else {
+                    for (int r = 0; r < rows; ++r) {
+                        T* g = gout + (base + r) * SP + BEGIN;
+                        for (int c = lane; c < LEN; c += 32) __stcs(g + c, tile[r * PITCH + c]);
+                    }
+                }
+                __syncwarp();
+            }
+        }
+    }
+};
+
+template <int KIND, int LMAX, typename T, typename TI, int CAP, int MODE, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32) sh_aos_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out) {
+    using Sink = RowSink<KIND, LMAX, T, CAP, MODE>;
+    static_assert(Sink::Seg::valid(), "CAP too small for one l-block group");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    T* tile = reinterpret_cast<T*>(smem_raw) + (size_t)warp * 32 * Sink::PITCH;
+    const int64_t ntiles = (n + 31) >> 5;
+    for (int64_t t = (int64_t)blockIdx.x * WARPS + warp; t < ntiles; t += (int64_t)gridDim.x * WARPS) {
+        const int64_t base = t << 5;
+        int64_t i = base + lane;
+        const int64_t left = n - base;
+        Sink sink;
+        sink.row = tile + lane * Sink::PITCH;
+        sink.tile = tile;
+        sink.gout = out;
+        sink.base = base;
+        sink.rows = left < 32 ? (int)left : 32;
+        sink.lane = lane;
+        if constexpr (MODE == MODE_ROWBULK) {
+            if (i >= n) continue;       // per-lane rows, no warp-level synchronization: idle lanes just skip
+            sink.wait_reads();          // previous tile's bulk copy has finished reading this row
+        } else {
+            if (i >= n) i = n - 1;      // all lanes take part in the copy-out; the clamped row is not written
+        }
+        sink.i = i;
+        const UnitVec u = load_unit(xyz, i);
+        evaluate<KIND, LMAX, T>(u, sink);
+    }
+    if constexpr (MODE == MODE_ROWBULK) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+
+// ------------------------------------------------------------------------------------------------
+// host side
+std::atomic<int64_t> g_launches{0};
+thread_local char g_cuda_error[256] = "";
+
+int cuda_fail(cudaError_t e) {
+    std::strncpy(g_cuda_error, cudaGetErrorString(e), sizeof(g_cuda_error) - 1);
+    return SH_ERR_CUDA;
+}
+
+int sm_count() {
+    static int sms = 0;
+    if (!sms) {
+        int dev = 0, v = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0)
+            sms = v;
+        else
+            return 148;
+    }
+    return sms;
+}
+
+template <int KIND, int LMAX, typename T, typename TI, int VEC>
+int launch_soa(const TI* xyz, int64_t n, T* out, cudaStream_t st) {
+    const int64_t blocks = (n + 255) / 256;
+    if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
+    sh_soa_kernel<KIND, LMAX, T, TI, VEC><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, out);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? SH_OK : cuda_fail(e);
+}
+
+// staging capacity per row, in scalars: whole rows for real (800 B at lmax = 9) and complex (1600 B);
+// spinor rows (6400 B) are staged in groups of l-blocks of at most 1600 B
+template <int KIND, int LMAX>
+constexpr int aos_cap() {
+    return KIND == KIND_SPINOR ? (200 > 8 * (2 * LMAX + 1) ? 200 : 8 * (2 * LMAX + 1)) : scalars_per_point(KIND, LMAX);
+}
+
+template <int KIND, int LMAX, typename T, typename TI, int MODE>
+int launch_aos(const TI* xyz, int64_t n, T* out, cudaStream_t st) {
+    constexpr int CAP = aos_cap<KIND, LMAX>();
+    constexpr int WARPS = 4;
+    using Sink = RowSink<KIND, LMAX, T, CAP, MODE>;
+    constexpr size_t smem = (size_t)WARPS * 32 * Sink::PITCH * sizeof(T);
+    static_assert(smem <= 227 * 1024, "staging tile exceeds shared memory");
+    auto kern = sh_aos_kernel<KIND, LMAX, T, TI, CAP, MODE, WARPS>;
+    static int ctas_per_sm = 0;   // idempotent cache of a pure function of the kernel
+    if (!ctas_per_sm) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return cuda_fail(e);
+        int occ = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, WARPS * 32, smem);
+        if (e != cudaSuccess) return cuda_fail(e);
+        ctas_per_sm = occ > 0 ? occ : 1;
+    }
+    const int64_t ntiles = (n + 31) / 32;
+    const int64_t want = (ntiles + WARPS - 1) / WARPS;
+    const int64_t resident = (int64_t)sm_count() * ctas_per_sm;
+    // persistent-style launch: every CTA stays resident and strides over the tiles
+    const int64_t blocks = want < resident ? want : resident;
+    kern<<<(unsigned)blocks, WARPS * 32, smem, st>>>(xyz, n, out);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? SH_OK : cuda_fail(e);
+}
+
+inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+template <int KIND, int LMAX, typename T, typename TI>
+int dispatch_lmax(const TI* xyz, int64_t n, T* out, int layout, int path, cudaStream_t st) {
+    constexpr int SP = scalars_per_point(KIND, LMAX);
+    if (layout == SH_LAYOUT_SOA) {
+        if (path == SH_STORE_BULK) return SH_ERR_ALIGNMENT;   // bulk path is AoS only
+        constexpr int ES = elem_scalars(KIND);
+        // plane e starts at out + e*n*ES scalars: vector stores need that to stay aligned for every e
+        const size_t plane_bytes = (size_t)n * ES * sizeof(T);
+        if (ES * sizeof(T) >= 32 && aligned(out, 32) && plane_bytes % 32 == 0) return launch_soa<KIND, LMAX, T, TI, 32>(xyz, n, out, st);
+        if (ES * sizeof(T) >= 16 && aligned(out, 16) && plane_bytes % 16 == 0) return launch_soa<KIND, LMAX, T, TI, 16>(xyz, n, out, st);
+        return launch_soa<KIND, LMAX, T, TI, 8>(xyz, n, out, st);
+    }
+    const bool bulk_ok = aligned(out, 16) && (SP * sizeof(T)) % 16 == 0;
+    if (path == SH_STORE_BULK && !bulk_ok) return SH_ERR_ALIGNMENT;
+    if constexpr ((SP * sizeof(T)) % 16 == 0) {
+        if (bulk_ok && path != SH_STORE_DIRECT) return launch_aos<KIND, LMAX, T, TI, MODE_ROWBULK>(xyz, n, out, st);
+    }
+    return launch_aos<KIND, LMAX, T, TI, MODE_PLAIN>(xyz, n, out, st);
+}
+
+template <int KIND, typename T, typename TI>
+int run_device(const TI* xyz, int64_t n, int lmax, T* out, int layout_bits, void* stream) {
+    if (n < 0) return SH_ERR_COUNT;
+    if (lmax < 0 || lmax > shgen::LMAX_CAP) return SH_ERR_LMAX;
+    const int layout = layout_bits & 0xff, path = layout_bits & 0xff00;
+    if ((layout_bits & ~0xffff) || (layout != SH_LAYOUT_AOS && layout != SH_LAYOUT_SOA) ||
+        (path != SH_STORE_AUTO && path != SH_STORE_DIRECT && path != SH_STORE_BULK))
+        return SH_ERR_LAYOUT;
+    if (n == 0) return SH_OK;
+    if (!xyz || !out) return SH_ERR_NULL;
+    if (!aligned(out, sizeof(T)) || !aligned(xyz, sizeof(TI))) return SH_ERR_ALIGNMENT;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    switch (lmax) {
+#define SH_CASE(L) case L: return dispatch_lmax<KIND, L, T, TI>(xyz, n, out, layout, path, st);
+        SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(3) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8) SH_CASE(9)
+#undef SH_CASE
+    }
+    return SH_ERR_LMAX;
+}
+
+// Host-buffer pipeline: chunks of points go host -> device -> kernel -> host on two streams (double buffering).
+template <int KIND, typename T, typename TI>
+int run_host(const TI* xyz, int64_t n, int lmax, T* out, int layout_bits) {
+    if (n < 0) return SH_ERR_COUNT;
+    if (lmax < 0 || lmax > shgen::LMAX_CAP) return SH_ERR_LMAX;
+    const int layout = layout_bits & 0xff;
+    if (layout != SH_LAYOUT_AOS && layout != SH_LAYOUT_SOA) return SH_ERR_LAYOUT;
+    if (n == 0) return SH_OK;
+    if (!xyz || !out) return SH_ERR_NULL;
+    const int64_t sp = (int64_t)elem_scalars(KIND) * elems_per_point(KIND, lmax);   // scalars per point
+    const int64_t es = elem_scalars(KIND), ne = sp / es;
+    // chunk: ~256 MiB of output per buffer, a multiple of 256 points, at least 256
+    int64_t chunk = ((int64_t)256 << 20) / (sp * (int64_t)sizeof(T));
+    chunk = chunk / 256 * 256;
+    if (chunk < 256) chunk = 256;
+    if (chunk > n) chunk = n;
+    cudaStream_t st[2] = {nullptr, nullptr};
+    TI* dxyz[2] = {nullptr, nullptr};
+    T* dout[2] = {nullptr, nullptr};
+    int rc = SH_OK;
+    auto check = [&](cudaError_t e) { if (e != cudaSuccess && rc == SH_OK) rc = cuda_fail(e); return e == cudaSuccess; };
+    const int nbuf = n > chunk ? 2 : 1;
+    for (int b = 0; b < nbuf && rc == SH_OK; ++b) {
+        check(cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking)) &&
+            check(cudaMalloc(&dxyz[b], (size_t)chunk * 3 * sizeof(TI))) && check(cudaMalloc(&dout[b], (size_t)chunk * sp * sizeof(T)));
+    }
+    for (int64_t c0 = 0, it = 0; c0 < n && rc == SH_OK; c0 += chunk, ++it) {
+        const int b = (int)(it % nbuf);
+        const int64_t m = (n - c0) < chunk ? (n - c0) : chunk;
+        if (!check(cudaMemcpyAsync(dxyz[b], xyz + 3 * c0, (size_t)m * 3 * sizeof(TI), cudaMemcpyHostToDevice, st[b]))) break;
+        int r = run_device<KIND, T, TI>(dxyz[b], m, lmax, dout[b], layout_bits, st[b]);
+        if (r != SH_OK) { rc = r; break; }
+        if (layout == SH_LAYOUT_AOS) {
+            check(cudaMemcpyAsync(out + c0 * sp, dout[b], (size_t)m * sp * sizeof(T), cudaMemcpyDeviceToHost, st[b]));
+        } else {
+            // device chunk is [ne][m] elements; host array is [ne][n]: one strided 2-D copy
+            check(cudaMemcpy2DAsync(out + c0 * es, (size_t)n * es * sizeof(T), dout[b], (size_t)m * es * sizeof(T),
+                                    (size_t)m * es * sizeof(T), (size_t)ne, cudaMemcpyDeviceToHost, st[b]));
+        }
+    }
+    for (int b = 0; b < nbuf; ++b) {
+        if (st[b]) { check(cudaStreamSynchronize(st[b])); cudaStreamDestroy(st[b]); }
+        if (dxyz[b]) cudaFree(dxyz[b]);
+        if (dout[b]) cudaFree(dout[b]);
+    }
+    return rc;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+extern "C" {
+
+int sh_real(const double* xyz, int64_t n, int lmax, double* out, int layout, void* stream) {
+    return run_device<KIND_REAL, double, double>(xyz, n, lmax, out, layout, stream);
+}
+int sh_complex(const double* xyz, int64_t n, int lmax, double* out, int layout, void* stream) {
+    return run_device<KIND_COMPLEX, double, double>(xyz, n, lmax, out, layout, stream);
+}
+int sh_spinor(const double* xyz, int64_t n, int lmax, double* out, int layout, void* stream) {
+    return run_device<KIND_SPINOR, double, double>(xyz, n, lmax, out, layout, stream);
+}
+int sh_real_f32(const float* xyz, int64_t n, int lmax, float* out, int layout, void* stream) {
+    return run_device<KIND_REAL, float, float>(xyz, n, lmax, out, layout, stream);
+}
+
+int sh_real_host(const double* xyz, int64_t n, int lmax, double* out, int layout) {
+    return run_host<KIND_REAL, double, double>(xyz, n, lmax, out, layout);
+}
+int sh_complex_host(const double* xyz, int64_t n, int lmax, double* out, int layout) {
+    return run_host<KIND_COMPLEX, double, double>(xyz, n, lmax, out, layout);
+}
+int sh_spinor_host(const double* xyz, int64_t n, int lmax, double* out, int layout) {
+    return run_host<KIND_SPINOR, double, double>(xyz, n, lmax, out, layout);
+}
+int sh_real_f32_host(const float* xyz, int64_t n, int lmax, float* out, int layout) {
+    return run_host<KIND_REAL, float, float>(xyz, n, lmax, out, layout);
+}
+
+int64_t sh_real_count(int lmax) { return (lmax < 0 || lmax > 9) ? -1 : (int64_t)(lmax + 1) * (lmax + 1); }
+int64_t sh_complex_count(int lmax) { return (lmax < 0 || lmax > 9) ? -1 : 2 * (int64_t)(lmax + 1) * (lmax + 1); }
+int64_t sh_spinor_count(int lmax) { return (lmax < 0 || lmax > 9) ? -1 : 8 * (int64_t)(lmax + 1) * (lmax + 1); }
+
+int sh_index_real(int l, int m) {
+    if (l < 0 || l > 9 || m < -l || m > l) return -1;
+    return l * (l + 1) + m;
+}
+
+int sh_index_spinor(int l, int twoj, int twomj) {
+    if (l < 0 || l > 9) return -1;
+    if (twoj != 2 * l - 1 && twoj != 2 * l + 1) return -1;
+    if (twoj < 1) return -1;
+    if (twomj < -twoj || twomj > twoj || ((twomj - twoj) & 1)) return -1;
+    const int off = (twomj + twoj) / 2;   // m_j + j
+    return 2 * l * l + (twoj == 2 * l - 1 ? off : 2 * l + off);
+}
+
+const char* sh_strerror(int code) {
+    switch (code) {
+        case SH_OK: return "ok";
+        case SH_ERR_NULL: return "xyz or out is NULL with n > 0";
+        case SH_ERR_COUNT: return "n is negative or too large for one launch";
+        case SH_ERR_LMAX: return "lmax must be in [0, 9]";
+        case SH_ERR_LAYOUT: return "unknown layout or store-path bits";
+        case SH_ERR_ALIGNMENT: return "pointer not aligned to its element type, or requested store path impossible for this alignment";
+        case SH_ERR_CUDA: return "CUDA error (see sh_last_cuda_error)";
+    }
+    return "unknown error code";
+}
+
+const char* sh_last_cuda_error(void) { return g_cuda_error; }
+int64_t sh_kernel_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+}  // extern "C"

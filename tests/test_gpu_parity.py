@@ -1,0 +1,297 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle on the
+same seeded inputs, element by element.  Tolerances are north_star's: max abs error 1e-12 in fp64,
+1e-5 for the fp32 variant.  Run on the B200 box: python -m pytest tests -m gpu.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-12
+TOL32 = 1e-5
+
+
+@pytest.fixture(scope="module")
+def sh():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2510_05282_b200 as pkg
+
+    pkg.load()  # raises if libshb200.so is missing: there is no fallback
+    return pkg
+
+
+def gpu_eval(sh, kind, xyz, lmax, layout, store="auto", misalign=0):
+    """Run the CUDA path; returns a numpy array in the oracle's AoS shape."""
+    import torch
+
+    dt = torch.float32 if kind == "real_f32" else torch.float64
+    x = torch.as_tensor(np.ascontiguousarray(xyz), dtype=dt).cuda()
+    n = x.shape[0]
+    shape = sh.out_shape(kind, n, lmax, layout)
+    numel = int(np.prod(shape))
+    backing = torch.full((numel + 8,), float("nan"), dtype=dt, device="cuda")
+    out = backing[misalign : misalign + numel]
+    fn = getattr(sh, "sh_" + kind)
+    fn(x, lmax, out=out, layout=layout, store=store)
+    torch.cuda.synchronize()
+    # guard elements around `out` untouched
+    assert torch.isnan(backing[:misalign]).all() and torch.isnan(backing[misalign + numel :]).all()
+    res = out.cpu().numpy().reshape(shape)
+    if layout == "soa":
+        res = np.moveaxis(res, 0, 1)  # [ne][n](...) -> [n][ne](...)
+    return np.ascontiguousarray(res)
+
+
+def oracle_eval(oracle_mod, kind, xyz, lmax):
+    if kind in ("real", "real_f32"):
+        return oracle_mod.real(np.asarray(xyz, dtype=np.float64), lmax)
+    if kind == "complex":
+        return oracle_mod.complex_(xyz, lmax).view(np.float64).reshape(len(xyz), -1, 2)
+    return oracle_mod.spinor(xyz, lmax).view(np.float64).reshape(len(xyz), -1, 4)
+
+
+def max_err(a, b):
+    return float(np.max(np.abs(a - b))) if a.size else 0.0
+
+
+# ----------------------------------------------------------------------------- config 1 and all (kind, lmax, layout, store)
+@pytest.fixture(scope="module")
+def cube_points():
+    from paper_2510_05282_b200 import inputs
+
+    return inputs.config1_cube()  # 10,008 points: 39 full 256-blocks + a ragged tail of 24; includes r = 0, poles, axes
+
+
+def test_config1_real_l4_soa(sh, oracle_mod, cube_points):
+    got = gpu_eval(sh, "real", cube_points, 4, "soa")
+    want = oracle_mod.real(cube_points, 4)
+    assert got.shape == (10008, 25)
+    assert max_err(got, want) <= TOL64
+    # r = 0 rows: exactly the convention
+    for row in (10000, 10007):
+        assert got[row, 0] == pytest.approx(0.28209479177387814, abs=1e-16) and np.all(got[row, 1:] == 0)
+
+
+@pytest.mark.parametrize("kind", ["real", "complex", "spinor"])
+@pytest.mark.parametrize("layout,store", [("soa", "auto"), ("aos", "auto"), ("aos", "direct")])
+def test_all_lmax_fp64(sh, oracle_mod, cube_points, kind, layout, store):
+    worst = 0.0
+    for lmax in range(10):
+        got = gpu_eval(sh, kind, cube_points, lmax, layout, store)
+        want = oracle_eval(oracle_mod, kind, cube_points, lmax)
+        assert got.shape == want.shape
+        worst = max(worst, max_err(got, want))
+    assert worst <= TOL64, worst
+
+
+@pytest.mark.parametrize("layout,store", [("soa", "auto"), ("aos", "auto"), ("aos", "direct")])
+def test_all_lmax_fp32(sh, oracle_mod, cube_points, layout, store):
+    x32 = cube_points.astype(np.float32)
+    for lmax in range(10):
+        got = gpu_eval(sh, "real_f32", x32, lmax, layout, store)
+        want = oracle_mod.real(x32.astype(np.float64), lmax)  # oracle at the fp32 inputs, converted exactly
+        assert max_err(got.astype(np.float64), want) <= TOL32, lmax
+
+
+def test_bulk_request_matches_and_is_refused_when_impossible(sh, oracle_mod, cube_points):
+    got = gpu_eval(sh, "real", cube_points, 9, "aos", "bulk")
+    assert max_err(got, oracle_mod.real(cube_points, 9)) <= TOL64
+    with pytest.raises(sh.ShError):  # K = 25 doubles per row: rows are not 16-byte multiples
+        gpu_eval(sh, "real", cube_points, 4, "aos", "bulk")
+    with pytest.raises(sh.ShError):  # bulk is an AoS path
+        gpu_eval(sh, "real", cube_points, 9, "soa", "bulk")
+    with pytest.raises(sh.ShError):  # 8-byte aligned out
+        gpu_eval(sh, "real", cube_points, 9, "aos", "bulk", misalign=1)
+
+
+@pytest.mark.parametrize("kind", ["real", "complex", "spinor"])
+@pytest.mark.parametrize("layout", ["soa", "aos"])
+def test_misaligned_out_and_odd_n_fall_back(sh, oracle_mod, kind, layout):
+    """8-byte aligned `out` and odd n (SoA planes lose 16/32-byte alignment): scalar paths, same values."""
+    from paper_2510_05282_b200 import inputs
+
+    pts = inputs.config1_cube(333, seed=4)[:-1]  # n = 340, then odd sizes below
+    for n in (340, 339, 33):
+        got = gpu_eval(sh, kind, pts[:n], 9, layout, "auto", misalign=1)
+        assert max_err(got, oracle_eval(oracle_mod, kind, pts[:n], 9)) <= TOL64, n
+    got = gpu_eval(sh, kind, pts[:339], 5, layout, "auto", misalign=0)
+    assert max_err(got, oracle_eval(oracle_mod, kind, pts[:339], 5)) <= TOL64
+
+
+@pytest.mark.parametrize("n", [0, 1, 31, 32, 33, 255, 256, 257])
+def test_small_and_ragged_sizes(sh, oracle_mod, n):
+    rng = np.random.default_rng(100 + n)
+    pts = rng.uniform(-2, 2, (n, 3))
+    for kind in ("real", "complex", "spinor"):
+        for layout in ("soa", "aos"):
+            got = gpu_eval(sh, kind, pts, 9, layout)
+            want = oracle_eval(oracle_mod, kind, pts, 9)
+            assert got.shape == want.shape and max_err(got, want) <= TOL64, (kind, layout)
+
+
+def test_extreme_radii_and_non_finite(sh, oracle_mod):
+    rng = np.random.default_rng(9)
+    d = rng.standard_normal((64, 3))
+    scales = np.array([1e-320, 1e-300, 1e-200, 1e-160, 1e-150, 1e-3, 1.0, 1e2, 1e150, 1e160, 1e200, 1e300])
+    pts = np.concatenate([d * s for s in scales])
+    for layout in ("soa", "aos"):
+        got = gpu_eval(sh, "real", pts, 9, layout)
+        want = oracle_mod.real(pts, 9)
+        # the oracle sees the same (possibly subnormal-rounded) inputs: same direction
+        assert max_err(got, want) <= TOL64
+    bad = np.array([[np.nan, 1.0, 2.0], [1.0, np.inf, 0.0], [-np.inf, np.inf, 1.0], [0.5, 0.5, 0.5]])
+    for layout in ("soa", "aos"):
+        got = gpu_eval(sh, "real", bad, 3, layout)
+        assert np.all(np.isnan(got[:3, 1:])) and np.all(np.isfinite(got[3]))
+
+
+def test_near_pole_points(sh, oracle_mod):
+    rng = np.random.default_rng(10)
+    pts = []
+    for s in (1e-2, 2.4e-4, 1e-5, 1e-7, 1e-9, 1e-12):
+        for _ in range(8):
+            phi = rng.uniform(-np.pi, np.pi)
+            pts.append([s * np.cos(phi), s * np.sin(phi), rng.choice([-1.0, 1.0])])
+    pts = np.array(pts) * 3.0
+    for kind in ("real", "complex", "spinor"):
+        got = gpu_eval(sh, kind, pts, 9, "soa")
+        assert max_err(got, oracle_eval(oracle_mod, kind, pts, 9)) <= TOL64
+
+
+# ----------------------------------------------------------------------------- config 2
+def test_config2_projector_grid(sh, oracle_mod):
+    from paper_2510_05282_b200 import inputs
+
+    pts = inputs.config2_projector_grid()
+    assert pts.shape == (113102, 3)
+    got = gpu_eval(sh, "real", pts, 3, "soa")
+    assert max_err(got, oracle_mod.real(pts, 3)) <= TOL64
+
+
+# ----------------------------------------------------------------------------- config 3 (headline), full size, every point
+@pytest.mark.parametrize("layout,store", [("soa", "auto"), ("aos", "auto"), ("aos", "direct")])
+def test_config3_full_grid_every_point(sh, oracle_mod, layout, store):
+    from paper_2510_05282_b200 import inputs
+
+    pts = inputs.config3_full_grid()
+    assert pts.shape == (128**3, 3)
+    got = gpu_eval(sh, "real", pts, 9, layout, store)
+    worst = 0.0
+    for lo in range(0, len(pts), 1 << 18):  # oracle in slabs to bound host memory
+        hi = min(len(pts), lo + (1 << 18))
+        worst = max(worst, max_err(got[lo:hi], oracle_mod.real(pts[lo:hi], 9)))
+    assert worst <= TOL64, worst
+
+
+# ----------------------------------------------------------------------------- configs 4 and 5: full size on the GPU, sampled + properties
+def sample_indices(n, k, seed):
+    rng = np.random.default_rng(seed)
+    idx = np.concatenate([np.arange(64), np.arange(n - 64, n), rng.integers(0, n, k)])
+    return np.unique(idx)
+
+
+def run_full(sh, kind, x, lmax, layout):
+    import torch
+
+    out = getattr(sh, "sh_" + kind)(x, lmax, layout=layout)
+    torch.cuda.synchronize()
+    return out
+
+
+@pytest.mark.parametrize("layout", ["soa", "aos"])
+def test_config4_complex_2pow24(sh, oracle_mod, layout):
+    import torch
+    from paper_2510_05282_b200 import inputs
+
+    pts = inputs.config4_sphere_directions()
+    n = len(pts)
+    assert n == 1 << 24
+    x = torch.from_numpy(pts).cuda()
+    out = run_full(sh, "complex", x, 9, layout)  # 26.8 GB
+    idx = sample_indices(n, 60000, 41)
+    tidx = torch.from_numpy(idx).cuda()
+    got = (out[:, tidx].permute(1, 0, 2) if layout == "soa" else out[tidx]).contiguous().cpu().numpy()
+    want = oracle_eval(oracle_mod, "complex", pts[idx], 9)
+    assert max_err(got, want) <= TOL64
+    # property at every point: sum_m |Y_l^m|^2 = (2l+1)/(4 pi)
+    worst = 0.0
+    for l in range(10):
+        sl = slice(l * l, (l + 1) ** 2)
+        blk = out[sl] if layout == "soa" else out[:, sl]
+        dens = (blk * blk).sum(dim=(0, 2)) if layout == "soa" else (blk * blk).sum(dim=(1, 2))
+        worst = max(worst, float((dens - (2 * l + 1) / (4 * np.pi)).abs().max()))
+        del blk, dens
+    assert worst <= 1e-13, worst
+
+
+@pytest.mark.parametrize("layout", ["soa", "aos"])
+def test_config5_spinor_2pow22(sh, oracle_mod, layout):
+    import torch
+    from paper_2510_05282_b200 import inputs
+
+    pts = inputs.config5_ball()
+    n = len(pts)
+    assert n == 1 << 22
+    x = torch.from_numpy(pts).cuda()
+    out = run_full(sh, "spinor", x, 9, layout)  # 26.8 GB
+    idx = sample_indices(n, 30000, 51)
+    tidx = torch.from_numpy(idx).cuda()
+    got = (out[:, tidx].permute(1, 0, 2) if layout == "soa" else out[tidx]).contiguous().cpu().numpy()
+    assert max_err(got, oracle_eval(oracle_mod, "spinor", pts[idx], 9)) <= TOL64
+    # property at every point: sum over the 2(2l+1) states of a given l of S^dagger S = 2 (2l+1)/(4 pi)
+    worst = 0.0
+    for l in range(10):
+        sl = slice(2 * l * l, 2 * (l + 1) ** 2)
+        blk = out[sl] if layout == "soa" else out[:, sl]
+        dens = (blk * blk).sum(dim=(0, 2)) if layout == "soa" else (blk * blk).sum(dim=(1, 2))
+        worst = max(worst, float((dens - 2 * (2 * l + 1) / (4 * np.pi)).abs().max()))
+        del blk, dens
+    assert worst <= 1e-13, worst
+
+
+@pytest.mark.parametrize("layout", ["soa", "aos"])
+def test_config5_real_f32_variant(sh, oracle_mod, layout):
+    import torch
+    from paper_2510_05282_b200 import inputs
+
+    pts32 = inputs.config5_ball().astype(np.float32)
+    n = len(pts32)
+    x = torch.from_numpy(pts32).cuda()
+    out = run_full(sh, "real_f32", x, 9, layout)
+    idx = sample_indices(n, 200000, 52)
+    tidx = torch.from_numpy(idx).cuda()
+    got = (out[:, tidx].t() if layout == "soa" else out[tidx]).contiguous().cpu().numpy().astype(np.float64)
+    want = oracle_mod.real(pts32[idx].astype(np.float64), 9)
+    assert max_err(got, want) <= TOL32
+
+
+# ----------------------------------------------------------------------------- host-buffer entry points
+@pytest.mark.parametrize("kind,lmax,n", [("real", 9, 400_000), ("complex", 4, 70_001), ("spinor", 3, 5_000), ("real_f32", 9, 10_008)])
+@pytest.mark.parametrize("layout", ["soa", "aos"])
+def test_host_entry_points(sh, oracle_mod, kind, lmax, n, layout):
+    rng = np.random.default_rng(77)
+    pts = rng.uniform(-3, 3, (n, 3))
+    if kind == "real_f32":
+        pts = pts.astype(np.float32)
+    got = sh.host_call(kind, pts, lmax, layout=layout)  # n = 400k at lmax 9: two pipeline chunks
+    if layout == "soa":
+        got = np.moveaxis(got, 0, 1)
+    want = oracle_eval(oracle_mod, kind, pts.astype(np.float64), lmax)
+    tol = TOL32 if kind == "real_f32" else TOL64
+    assert max_err(np.asarray(got, dtype=np.float64).reshape(want.shape), want) <= tol
+
+
+def test_launch_counter_and_streams(sh, oracle_mod, cube_points):
+    import torch
+
+    before = sh.kernel_launch_count()
+    x = torch.from_numpy(cube_points).cuda()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        out = sh.sh_real(x, 9, layout="aos")
+    s.synchronize()
+    assert sh.kernel_launch_count() == before + 1
+    assert max_err(out.cpu().numpy(), oracle_mod.real(cube_points, 9)) <= TOL64

@@ -1,0 +1,87 @@
+"""CPU-side checks of the C-ABI library: it loads, exports every symbol include/shb200.h declares,
+and validates arguments before touching the GPU.  No kernel is launched here."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2510_05282_b200 import build, binding
+
+    build.build()
+    return binding.load()
+
+
+def declared_functions():
+    text = open(os.path.join(ROOT, "include", "shb200.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(sh_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_header_symbols_are_exported(lib):
+    names = declared_functions()
+    assert len(names) >= 16 and "sh_real" in names and "sh_spinor_host" in names
+    for name in names:
+        assert hasattr(lib, name), name
+
+
+def test_counts_and_indices(lib):
+    for lmax in range(10):
+        k = (lmax + 1) ** 2
+        assert lib.sh_real_count(lmax) == k and lib.sh_complex_count(lmax) == 2 * k and lib.sh_spinor_count(lmax) == 8 * k
+    assert lib.sh_real_count(10) == -1 and lib.sh_spinor_count(-1) == -1
+    assert [lib.sh_index_real(l, m) for l in range(10) for m in range(-l, l + 1)] == list(range(100))
+    assert lib.sh_index_real(3, 4) == -1 and lib.sh_index_real(10, 0) == -1
+    seen = []
+    for l in range(10):
+        for twoj in (2 * l - 1, 2 * l + 1):
+            if twoj < 1:
+                continue
+            seen += [lib.sh_index_spinor(l, twoj, tm) for tm in range(-twoj, twoj + 1, 2)]
+    assert seen == list(range(200))
+    assert lib.sh_index_spinor(0, -1, 1) == -1 and lib.sh_index_spinor(2, 5, 4) == -1 and lib.sh_index_spinor(2, 5, 7) == -1
+
+
+def test_argument_validation_without_gpu(lib):
+    """Errors are returned before any CUDA call (P: boundary contract in include/shb200.h)."""
+    buf = np.zeros(64, dtype=np.float64)
+    p = buf.ctypes.data
+    for fn in (lib.sh_real, lib.sh_complex, lib.sh_spinor, lib.sh_real_f32):
+        assert fn(p, -1, 3, p, 0, None) == -2            # SH_ERR_COUNT
+        assert fn(p, 4, 10, p, 0, None) == -3            # SH_ERR_LMAX
+        assert fn(p, 4, -1, p, 1, None) == -3
+        assert fn(p, 4, 3, p, 2, None) == -4             # SH_ERR_LAYOUT
+        assert fn(p, 4, 3, p, 0 | (3 << 8), None) == -4
+        assert fn(None, 4, 3, p, 0, None) == -1          # SH_ERR_NULL
+        assert fn(p, 4, 3, None, 1, None) == -1
+        assert fn(None, 0, 3, None, 0, None) == 0        # n = 0: successful no-op
+    assert lib.sh_real(p, 4, 3, p + 4, 0, None) == -5    # SH_ERR_ALIGNMENT
+    for fn in (lib.sh_real_host, lib.sh_complex_host, lib.sh_spinor_host, lib.sh_real_f32_host):
+        assert fn(p, -1, 3, p, 0) == -2 and fn(p, 1, 11, p, 0) == -3 and fn(None, 0, 3, None, 1) == 0
+    for code in range(-6, 1):
+        assert len(lib.sh_strerror(code)) > 1
+    assert lib.sh_strerror(-99) == b"unknown error code"
+
+
+def test_binding_fails_loudly_without_library(monkeypatch, tmp_path):
+    from paper_2510_05282_b200 import binding
+
+    monkeypatch.setattr(binding, "_lib", None)
+    monkeypatch.setattr(binding, "LIB_PATH", str(tmp_path / "missing.so"))
+    with pytest.raises(FileNotFoundError):
+        binding.load()
+
+
+def test_generator_output_is_current():
+    """csrc/sh_generated.cuh is exactly what the generator emits (committed copy is not stale)."""
+    from paper_2510_05282_b200.gen import generate
+
+    generate.self_check()
+    path = os.path.join(ROOT, "paper_2510_05282_b200", "csrc", "sh_generated.cuh")
+    assert open(path).read() == generate.emit()
