@@ -99,6 +99,15 @@ int sh_index_real(int l, int m);
  * -1 if the triple is not a valid spin-1/2 state with l <= 9. */
 int sh_index_spinor(int l, int twoj, int twomj);
 
+/* Launch-heuristic overrides, for benchmarking and tuning only: process-global, do not change results.
+ * value 0 restores the built-in default; returns SH_ERR_LAYOUT for an unknown knob or a negative value. */
+enum {
+    SH_TUNE_SOA_TILES_PER_CTA = 0,  /* consecutive 256-point tiles one CTA of the SoA kernels processes */
+    SH_TUNE_AOS_TILES_PER_WARP = 1, /* consecutive 32-point tiles one warp of the AoS kernels processes */
+    SH_TUNE_COUNT = 2
+};
+int sh_set_tuning(int knob, int value);
+
 /* Static text for an SH_ERR_* code. */
 const char* sh_strerror(int code);
 /* Text of the last CUDA error seen by this thread's calls ("" if none). */

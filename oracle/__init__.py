@@ -79,7 +79,7 @@ def complex_(xyz, lmax):
 
 def spinor(xyz, lmax):
     """Spin-1/2 spinor harmonics at Cartesian points: [n][2K][2] complex128 (up, down)."""
-    return _call("spinor", xyz, 3, lmax, 8 * count(lmax)).view(np.complex128).reshape(-1, 2 * count(lmax), 2)
+    return _call("spinor", xyz, 3, lmax, 8 * count(lmax)).view(np.complex128).reshape(len(xyz), 2 * count(lmax), 2)
 
 
 def real_angular(theta_phi, lmax):
@@ -92,7 +92,7 @@ def complex_angular(theta_phi, lmax):
 
 def spinor_angular(theta_phi, lmax):
     return _call("spinor_angular", theta_phi, 2, lmax, 8 * count(lmax)).view(np.complex128).reshape(
-        -1, 2 * count(lmax), 2
+        len(theta_phi), 2 * count(lmax), 2
     )
 
 

@@ -74,11 +74,17 @@ __device__ __forceinline__ UnitVec normalize(double x, double y, double z) {
     return u;
 }
 
+// a1: one point of the AoS input.  Loaded one tile ahead of its use (software prefetch): under a saturated
+// write stream the read latency is several microseconds, and nothing else in a warp's tile depends on memory.
 template <typename TI>
-__device__ __forceinline__ UnitVec load_unit(const TI* __restrict__ xyz, int64_t i) {
-    const TI* p = xyz + 3 * i;
-    return normalize((double)__ldg(p), (double)__ldg(p + 1), (double)__ldg(p + 2));
-}
+struct RawPoint {
+    TI x, y, z;
+    __device__ __forceinline__ void load(const TI* __restrict__ xyz, int64_t i) {
+        const TI* p = xyz + 3 * i;
+        x = __ldg(p); y = __ldg(p + 1); z = __ldg(p + 2);
+    }
+    __device__ __forceinline__ UnitVec unit() const { return normalize((double)x, (double)y, (double)z); }
+};
 
 // ------------------------------------------------------------------------------------------------
 // a3-a7: evaluators.  Sink interface: put1<K>(v) real element K; put2<K>(re, im) complex element K;
@@ -226,13 +232,25 @@ struct SoASink {
 };
 
 template <int KIND, int LMAX, typename T, typename TI, int VEC>
-__global__ void __launch_bounds__(256) sh_soa_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out) {
-    const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
-    if (i >= n) return;
-    const UnitVec u = load_unit(xyz, i);
+__global__ void __launch_bounds__(256) sh_soa_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out, int tiles_per_cta) {
     constexpr int ES = elem_scalars(KIND);
-    SoASink<T, VEC> sink{out + i * ES, n * ES};
-    evaluate<KIND, LMAX, T>(u, sink);
+    const int64_t ntiles = (n + 255) >> 8;
+    int64_t t = (int64_t)blockIdx.x * tiles_per_cta;
+    const int64_t tend = (t + tiles_per_cta < ntiles) ? t + tiles_per_cta : ntiles;
+    int64_t i = (t << 8) + threadIdx.x;
+    RawPoint<TI> cur, nxt;
+    bool have = i < n;
+    if (have) cur.load(xyz, i);
+    for (; t < tend; ++t, i += 256) {
+        const bool have_next = (t + 1 < tend) && (i + 256 < n);
+        if (have_next) nxt.load(xyz, i + 256);
+        if (have) {
+            SoASink<T, VEC> sink{out + i * ES, n * ES};
+            evaluate<KIND, LMAX, T>(cur.unit(), sink);
+        }
+        cur = nxt;
+        have = have_next;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -377,33 +395,43 @@ struct RowSink {
 };
 
 template <int KIND, int LMAX, typename T, typename TI, int CAP, int MODE, int WARPS>
-__global__ void __launch_bounds__(WARPS * 32) sh_aos_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out) {
+__global__ void __launch_bounds__(WARPS * 32) sh_aos_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out, int tiles_per_warp) {
     using Sink = RowSink<KIND, LMAX, T, CAP, MODE>;
     static_assert(Sink::Seg::valid(), "CAP too small for one l-block group");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     T* tile = reinterpret_cast<T*>(smem_raw) + (size_t)warp * 32 * Sink::PITCH;
     const int64_t ntiles = (n + 31) >> 5;
-    for (int64_t t = (int64_t)blockIdx.x * WARPS + warp; t < ntiles; t += (int64_t)gridDim.x * WARPS) {
-        const int64_t base = t << 5;
-        int64_t i = base + lane;
-        const int64_t left = n - base;
-        Sink sink;
-        sink.row = tile + lane * Sink::PITCH;
-        sink.tile = tile;
-        sink.gout = out;
-        sink.base = base;
-        sink.rows = left < 32 ? (int)left : 32;
-        sink.lane = lane;
-        if constexpr (MODE == MODE_ROWBULK) {
-            if (i >= n) continue;       // per-lane rows, no warp-level synchronization: idle lanes just skip
-            sink.wait_reads();          // previous tile's bulk copy has finished reading this row
-        } else {
-            if (i >= n) i = n - 1;      // all lanes take part in the copy-out; the clamped row is not written
+    // warp w of CTA b owns tiles [(b*WARPS + w) * tiles_per_warp, +tiles_per_warp): a contiguous span of `out`
+    int64_t t = ((int64_t)blockIdx.x * WARPS + warp) * tiles_per_warp;
+    const int64_t tend = (t + tiles_per_warp < ntiles) ? t + tiles_per_warp : ntiles;
+    // plain mode: every lane takes part in the copy-out, so idle lanes of the last tile evaluate a clamped point
+    auto point_of = [&](int64_t tt) {
+        const int64_t i = (tt << 5) + lane;
+        return (MODE == MODE_PLAIN && i >= n) ? n - 1 : i;
+    };
+    RawPoint<TI> cur, nxt;
+    bool have = t < tend && point_of(t) < n;
+    if (have) cur.load(xyz, point_of(t));
+    for (; t < tend; ++t) {
+        const bool have_next = (t + 1 < tend) && point_of(t + 1) < n;
+        if (have_next) nxt.load(xyz, point_of(t + 1));
+        if (have) {
+            const int64_t base = t << 5;
+            const int64_t left = n - base;
+            Sink sink;
+            sink.row = tile + lane * Sink::PITCH;
+            sink.tile = tile;
+            sink.gout = out;
+            sink.base = base;
+            sink.rows = left < 32 ? (int)left : 32;
+            sink.lane = lane;
+            sink.i = point_of(t);
+            sink.wait_reads();   // bulk mode: the previous tile's copy has finished reading this lane's row
+            evaluate<KIND, LMAX, T>(cur.unit(), sink);
         }
-        sink.i = i;
-        const UnitVec u = load_unit(xyz, i);
-        evaluate<KIND, LMAX, T>(u, sink);
+        cur = nxt;
+        have = have_next;
     }
     if constexpr (MODE == MODE_ROWBULK) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
@@ -430,11 +458,24 @@ int sm_count() {
     return sms;
 }
 
+// launch-heuristic overrides (sh_set_tuning); 0 = default
+std::atomic<int> g_tune[8];
+
+int tuned(int knob, int dflt) {
+    const int v = g_tune[knob].load(std::memory_order_relaxed);
+    return v > 0 ? v : dflt;
+}
+
 template <int KIND, int LMAX, typename T, typename TI, int VEC>
 int launch_soa(const TI* xyz, int64_t n, T* out, cudaStream_t st) {
-    const int64_t blocks = (n + 255) / 256;
+    const int64_t tiles = (n + 255) / 256;
+    // a few consecutive 256-point tiles per CTA so that the next tile's input load overlaps this tile's stores,
+    // while the grid stays many waves deep (the hardware CTA scheduler balances the SMs)
+    int tpc = tuned(SH_TUNE_SOA_TILES_PER_CTA, 2);
+    while (tpc > 1 && tiles / tpc < (int64_t)sm_count() * 16) tpc >>= 1;
+    const int64_t blocks = (tiles + tpc - 1) / tpc;
     if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
-    sh_soa_kernel<KIND, LMAX, T, TI, VEC><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, out);
+    sh_soa_kernel<KIND, LMAX, T, TI, VEC><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, out, tpc);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? SH_OK : cuda_fail(e);
@@ -465,11 +506,13 @@ int launch_aos(const TI* xyz, int64_t n, T* out, cudaStream_t st) {
         ctas_per_sm = occ > 0 ? occ : 1;
     }
     const int64_t ntiles = (n + 31) / 32;
-    const int64_t want = (ntiles + WARPS - 1) / WARPS;
-    const int64_t resident = (int64_t)sm_count() * ctas_per_sm;
-    // persistent-style launch: every CTA stays resident and strides over the tiles
-    const int64_t blocks = want < resident ? want : resident;
-    kern<<<(unsigned)blocks, WARPS * 32, smem, st>>>(xyz, n, out);
+    // a few consecutive tiles per warp (input prefetch across tiles, staging rows reused), many CTAs per SM over the
+    // run so that the hardware CTA scheduler evens out SM-to-SM speed differences
+    int tpw = tuned(SH_TUNE_AOS_TILES_PER_WARP, 4);
+    while (tpw > 1 && ntiles / ((int64_t)WARPS * tpw) < (int64_t)sm_count() * ctas_per_sm * 4) tpw >>= 1;
+    const int64_t blocks = (ntiles + (int64_t)WARPS * tpw - 1) / ((int64_t)WARPS * tpw);
+    if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
+    kern<<<(unsigned)blocks, WARPS * 32, smem, st>>>(xyz, n, out, tpw);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? SH_OK : cuda_fail(e);
@@ -485,8 +528,12 @@ int dispatch_lmax(const TI* xyz, int64_t n, T* out, int layout, int path, cudaSt
         constexpr int ES = elem_scalars(KIND);
         // plane e starts at out + e*n*ES scalars: vector stores need that to stay aligned for every e
         const size_t plane_bytes = (size_t)n * ES * sizeof(T);
-        if (ES * sizeof(T) >= 32 && aligned(out, 32) && plane_bytes % 32 == 0) return launch_soa<KIND, LMAX, T, TI, 32>(xyz, n, out, st);
-        if (ES * sizeof(T) >= 16 && aligned(out, 16) && plane_bytes % 16 == 0) return launch_soa<KIND, LMAX, T, TI, 16>(xyz, n, out, st);
+        if constexpr (ES * sizeof(T) >= 32) {
+            if (aligned(out, 32) && plane_bytes % 32 == 0) return launch_soa<KIND, LMAX, T, TI, 32>(xyz, n, out, st);
+        }
+        if constexpr (ES * sizeof(T) >= 16) {
+            if (aligned(out, 16) && plane_bytes % 16 == 0) return launch_soa<KIND, LMAX, T, TI, 16>(xyz, n, out, st);
+        }
         return launch_soa<KIND, LMAX, T, TI, 8>(xyz, n, out, st);
     }
     const bool bulk_ok = aligned(out, 16) && (SP * sizeof(T)) % 16 == 0;
@@ -511,7 +558,10 @@ int run_device(const TI* xyz, int64_t n, int lmax, T* out, int layout_bits, void
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     switch (lmax) {
 #define SH_CASE(L) case L: return dispatch_lmax<KIND, L, T, TI>(xyz, n, out, layout, path, st);
-        SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(3) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8) SH_CASE(9)
+#ifndef SHB200_DEV_ONLY_LMAX9   /* development builds may compile the lmax = 9 kernels only */
+        SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(3) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8)
+#endif
+        SH_CASE(9)
 #undef SH_CASE
     }
     return SH_ERR_LMAX;
@@ -628,6 +678,12 @@ const char* sh_strerror(int code) {
 }
 
 const char* sh_last_cuda_error(void) { return g_cuda_error; }
+
+int sh_set_tuning(int knob, int value) {
+    if (knob < 0 || knob >= SH_TUNE_COUNT || value < 0) return SH_ERR_LAYOUT;
+    g_tune[knob].store(value, std::memory_order_relaxed);
+    return SH_OK;
+}
 int64_t sh_kernel_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 }  // extern "C"

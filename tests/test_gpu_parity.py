@@ -48,9 +48,10 @@ def gpu_eval(sh, kind, xyz, lmax, layout, store="auto", misalign=0):
 def oracle_eval(oracle_mod, kind, xyz, lmax):
     if kind in ("real", "real_f32"):
         return oracle_mod.real(np.asarray(xyz, dtype=np.float64), lmax)
+    k = (lmax + 1) ** 2
     if kind == "complex":
-        return oracle_mod.complex_(xyz, lmax).view(np.float64).reshape(len(xyz), -1, 2)
-    return oracle_mod.spinor(xyz, lmax).view(np.float64).reshape(len(xyz), -1, 4)
+        return oracle_mod.complex_(xyz, lmax).view(np.float64).reshape(len(xyz), k, 2)
+    return oracle_mod.spinor(xyz, lmax).view(np.float64).reshape(len(xyz), 2 * k, 4)
 
 
 def max_err(a, b):
