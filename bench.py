@@ -217,11 +217,10 @@ def run_ours(args):
     import torch.distributed as dist
 
     import paper_2510_05282_b200 as sh
+    from paper_2510_05282_b200.dist import env_world, max_over_ranks
 
     sh.load()  # no fallback: fails here if libshb200.so is missing
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, local, world = env_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the CUDA path has no CPU fallback)")
     torch.cuda.set_device(local)
@@ -283,10 +282,7 @@ def run_ours(args):
     if clocks is not None:
         clocks["window"] = "timed region + untimed continuation of the same step loop, 1.5 s in total"
     ms = start.elapsed_time(end)
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dev)
     t_soa = sum(a.elapsed_time(b) for a, b, _ in marks) / len(marks)
     t_aos = sum(b.elapsed_time(c) for _, b, c in marks) / len(marks)
 
@@ -306,10 +302,7 @@ def run_ours(args):
     for _ in range(e2e_steps):
         e2e_step()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, dev)
     # spot-check the end-to-end result against the device-resident result
     assert torch.equal(h_aos[:1000], out_aos[(args.steps - 1) % nrep_out][:1000].cpu())
 
