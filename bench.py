@@ -173,7 +173,7 @@ def extra_configs(sh, dev):
     from paper_2510_05282_b200 import inputs
 
     def timed(fn, reps):
-        for _ in range(2):
+        for _ in range(3):
             fn()
         torch.cuda.synchronize()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -190,7 +190,7 @@ def extra_configs(sh, dev):
         ("config2 real l3 SoA N=113102", "real", inputs.config2_projector_grid(), 3, ["soa"], 50),
         ("config4 complex l9 N=2^24", "complex", inputs.config4_sphere_directions(), 9, ["soa", "aos"], 3),
         ("config5 spinor l9 N=2^22", "spinor", inputs.config5_ball(), 9, ["soa", "aos"], 3),
-        ("config5 real_f32 l9 N=2^22", "real_f32", inputs.config5_ball().astype(np.float32), 9, ["soa", "aos"], 5),
+        ("config5 real_f32 l9 N=2^22", "real_f32", inputs.config5_ball().astype(np.float32), 9, ["soa", "aos"], 20),
     ]
     for name, kind, pts, lmax, layouts, reps in cases:
         x = torch.from_numpy(pts).to(dev)

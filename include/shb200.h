@@ -60,12 +60,25 @@ enum {
     SH_STORE_BULK   = 2 << 8  /* AoS only: per-point rows staged in shared memory, written by TMA bulk copies (cp.async.bulk) */
 };
 
+/* Input front end, OR-ed into `layout` (bits 16-17).  Default: Cartesian.
+ *   SH_COORDS_CARTESIAN   xyz is [n][3] points of any norm; the library divides by r.
+ *   SH_COORDS_NORMALIZED  xyz is [n][3] UNIT vectors (Eq. 8, the paper's fastest interface): the normalization step is
+ *                         skipped; values are unspecified polynomials if the input is not normalized; a zero
+ *                         vector selects the r = 0 convention.
+ *   SH_COORDS_ANGULAR     xyz is [n][2] = (theta, phi), polar angle first (Eq. 3-4); x = sin(theta)cos(phi),
+ *                         y = sin(theta)sin(phi), z = cos(theta). */
+enum {
+    SH_COORDS_CARTESIAN  = 0 << 16,
+    SH_COORDS_NORMALIZED = 1 << 16,
+    SH_COORDS_ANGULAR    = 2 << 16
+};
+
 enum {
     SH_OK = 0,
     SH_ERR_NULL = -1,      /* xyz or out is NULL with n > 0 */
     SH_ERR_COUNT = -2,     /* n < 0 */
     SH_ERR_LMAX = -3,      /* lmax outside [0, 9] */
-    SH_ERR_LAYOUT = -4,    /* unknown layout or store-path bits */
+    SH_ERR_LAYOUT = -4,    /* unknown layout, store-path or front-end bits */
     SH_ERR_ALIGNMENT = -5, /* out not aligned to its element type, or requested store path not possible */
     SH_ERR_CUDA = -6       /* CUDA launch / copy error; text via sh_last_cuda_error() */
 };

@@ -16,6 +16,11 @@ SH_STORE_AUTO = 0 << 8
 SH_STORE_DIRECT = 1 << 8
 SH_STORE_BULK = 2 << 8
 
+SH_COORDS_CARTESIAN = 0 << 16
+SH_COORDS_NORMALIZED = 1 << 16
+SH_COORDS_ANGULAR = 2 << 16
+
+_COORDS = {"cartesian": SH_COORDS_CARTESIAN, "normalized": SH_COORDS_NORMALIZED, "angular": SH_COORDS_ANGULAR}
 _LAYOUTS = {"aos": SH_LAYOUT_AOS, "soa": SH_LAYOUT_SOA, SH_LAYOUT_AOS: SH_LAYOUT_AOS, SH_LAYOUT_SOA: SH_LAYOUT_SOA}
 _STORES = {"auto": SH_STORE_AUTO, "direct": SH_STORE_DIRECT, "bulk": SH_STORE_BULK}
 
@@ -65,8 +70,8 @@ def load() -> ctypes.CDLL:
     return _lib
 
 
-def layout_bits(layout, store="auto") -> int:
-    return _LAYOUTS[layout] | _STORES[store]
+def layout_bits(layout, store="auto", coords="cartesian") -> int:
+    return _LAYOUTS[layout] | _STORES[store] | _COORDS[coords]
 
 
 def count(kind: str, lmax: int) -> int:
@@ -96,13 +101,14 @@ def out_shape(kind: str, n: int, lmax: int, layout) -> tuple:
     return (ne, n, es) if es > 1 else (ne, n)
 
 
-def _device_call(kind: str, xyz, lmax: int, out, layout, store, stream):
+def _device_call(kind: str, xyz, lmax: int, out, layout, store, stream, coords="cartesian"):
     import torch
 
     fn = getattr(load(), "sh_" + kind)
     want = torch.float32 if kind == "real_f32" else torch.float64
-    if not (xyz.is_cuda and xyz.dtype == want and xyz.is_contiguous() and xyz.dim() == 2 and xyz.shape[1] == 3):
-        raise ValueError("xyz must be a contiguous CUDA tensor [n][3] of " + str(want))
+    width = 2 if coords == "angular" else 3
+    if not (xyz.is_cuda and xyz.dtype == want and xyz.is_contiguous() and xyz.dim() == 2 and xyz.shape[1] == width):
+        raise ValueError(f"xyz must be a contiguous CUDA tensor [n][{width}] of {want}")
     n = xyz.shape[0]
     shape = out_shape(kind, n, lmax, layout)
     if out is None:
@@ -111,33 +117,34 @@ def _device_call(kind: str, xyz, lmax: int, out, layout, store, stream):
         raise ValueError(f"out must be a contiguous CUDA tensor of {want} with {int(np.prod(shape))} elements")
     s = torch.cuda.current_stream(xyz.device).cuda_stream if stream is None else int(stream)
     with torch.cuda.device(xyz.device):
-        rc = fn(xyz.data_ptr(), n, int(lmax), out.data_ptr(), layout_bits(layout, store), s)
+        rc = fn(xyz.data_ptr(), n, int(lmax), out.data_ptr(), layout_bits(layout, store, coords), s)
     if rc != 0:
         raise ShError(rc, "sh_" + kind)
     return out
 
 
-def sh_real(xyz, lmax, out=None, layout="soa", store="auto", stream=None):
-    """R_l^m (Eq. 6) for l <= lmax at CUDA tensor xyz [n][3] float64 -> AoS [n][K] or SoA [K][n]."""
-    return _device_call("real", xyz, lmax, out, layout, store, stream)
+def sh_real(xyz, lmax, out=None, layout="soa", store="auto", stream=None, coords="cartesian"):
+    """R_l^m (Eq. 6) for l <= lmax at CUDA tensor xyz [n][3] float64 -> AoS [n][K] or SoA [K][n].
+    coords: "cartesian" (default), "normalized" (unit vectors, no normalization) or "angular" ([n][2] = theta, phi)."""
+    return _device_call("real", xyz, lmax, out, layout, store, stream, coords)
 
 
-def sh_complex(xyz, lmax, out=None, layout="soa", store="auto", stream=None):
+def sh_complex(xyz, lmax, out=None, layout="soa", store="auto", stream=None, coords="cartesian"):
     """Y_l^m (Eq. 5) -> AoS [n][K][2] or SoA [K][n][2] float64 (re, im)."""
-    return _device_call("complex", xyz, lmax, out, layout, store, stream)
+    return _device_call("complex", xyz, lmax, out, layout, store, stream, coords)
 
 
-def sh_spinor(xyz, lmax, out=None, layout="soa", store="auto", stream=None):
+def sh_spinor(xyz, lmax, out=None, layout="soa", store="auto", stream=None, coords="cartesian"):
     """Spinor harmonics (Eq. 7) -> AoS [n][2K][4] or SoA [2K][n][4] float64 (up.re, up.im, down.re, down.im)."""
-    return _device_call("spinor", xyz, lmax, out, layout, store, stream)
+    return _device_call("spinor", xyz, lmax, out, layout, store, stream, coords)
 
 
-def sh_real_f32(xyz, lmax, out=None, layout="soa", store="auto", stream=None):
+def sh_real_f32(xyz, lmax, out=None, layout="soa", store="auto", stream=None, coords="cartesian"):
     """fp32 variant of sh_real (float32 in, float32 out)."""
-    return _device_call("real_f32", xyz, lmax, out, layout, store, stream)
+    return _device_call("real_f32", xyz, lmax, out, layout, store, stream, coords)
 
 
-def host_call(kind: str, xyz: "np.ndarray | object", lmax: int, out=None, layout="soa"):
+def host_call(kind: str, xyz: "np.ndarray | object", lmax: int, out=None, layout="soa", coords="cartesian"):
     """sh_*_host: HOST buffers in and out (numpy arrays or CPU torch tensors, ideally pinned)."""
     fn = getattr(load(), f"sh_{kind}_host")
     dt = np.float32 if kind == "real_f32" else np.float64
@@ -154,7 +161,7 @@ def host_call(kind: str, xyz: "np.ndarray | object", lmax: int, out=None, layout
     if out is None:
         out = np.empty(shape, dtype=dt)
     op, ok = ptr_n(out)
-    rc = fn(xp, n, int(lmax), op, _LAYOUTS[layout])
+    rc = fn(xp, n, int(lmax), op, _LAYOUTS[layout] | _COORDS[coords])
     if rc != 0:
         raise ShError(rc, f"sh_{kind}_host")
     return ok

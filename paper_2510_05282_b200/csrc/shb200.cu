@@ -23,6 +23,7 @@
 #include <type_traits>
 
 #include "../../include/shb200.h"
+#define SHGEN_FN __device__ __forceinline__
 #include "sh_generated.cuh"
 
 namespace {
@@ -39,6 +40,28 @@ __device__ __forceinline__ void static_for(F&& f) {
         static_for<B + 1, E>(f);
     }
 }
+
+// ------------------------------------------------------------------------------------------------
+// f2: two fp32 lanes = two POINTS per thread, on Blackwell's packed-fp32 pipe (PTX fma/mul/add .f32x2, SASS
+// FFMA2/FMUL2/FADD2, sm_100+): one issue slot does the arithmetic of two points.  The generated templates are
+// written against a generic T, so T = f2 needs only these operators.
+struct f2 {
+    float2 v;
+    f2() = default;
+    __device__ __forceinline__ explicit f2(float a, float b) : v(make_float2(a, b)) {}
+    __device__ __forceinline__ explicit f2(double s) : v(make_float2((float)s, (float)s)) {}
+    __device__ __forceinline__ explicit f2(int s) : v(make_float2((float)s, (float)s)) {}
+};
+__device__ __forceinline__ f2 operator*(f2 a, f2 b) { f2 r; r.v = __fmul2_rn(a.v, b.v); return r; }
+__device__ __forceinline__ f2 operator+(f2 a, f2 b) { f2 r; r.v = __fadd2_rn(a.v, b.v); return r; }
+__device__ __forceinline__ f2 operator-(f2 a, f2 b) { f2 r; r.v = __ffma2_rn(b.v, make_float2(-1.f, -1.f), a.v); return r; }  // exact: one rounding
+__device__ __forceinline__ f2 operator-(f2 a) { return f2(-a.v.x, -a.v.y); }
+
+// r = 0 flags of the point(s) a thread evaluates, and "zero where the point is the origin"
+struct Origin2 { bool a, b; };
+__device__ __forceinline__ double zero_where(bool o, double q) { return o ? 0.0 : q; }
+__device__ __forceinline__ float zero_where(bool o, float q) { return o ? 0.f : q; }
+__device__ __forceinline__ f2 zero_where(Origin2 o, f2 q) { return f2(o.a ? 0.f : q.v.x, o.b ? 0.f : q.v.y); }
 
 // scalars (T) per element, elements per point
 __host__ __device__ constexpr int elem_scalars(int kind) { return kind == KIND_REAL ? 1 : kind == KIND_COMPLEX ? 2 : 4; }
@@ -74,16 +97,48 @@ __device__ __forceinline__ UnitVec normalize(double x, double y, double z) {
     return u;
 }
 
+// Normalized-Cartesian front end (the paper's fastest interface): the caller guarantees x^2+y^2+z^2 = 1
+// (Eq. 8); a2 is skipped.  A zero vector selects the r = 0 convention.
+__device__ __forceinline__ UnitVec as_given(double x, double y, double z) {
+    UnitVec u;
+    u.x = x; u.y = y; u.z = z;
+    u.origin = (x == 0.0 && y == 0.0 && z == 0.0);
+    return u;
+}
+
+// Angular front end: x = sin(theta) cos(phi), y = sin(theta) sin(phi), z = cos(theta).
+__device__ __forceinline__ UnitVec from_angles(double theta, double phi) {
+    double st, ct, sp, cp;
+    sincos(theta, &st, &ct);
+    sincos(phi, &sp, &cp);
+    UnitVec u;
+    u.x = st * cp; u.y = st * sp; u.z = ct;
+    u.origin = false;
+    return u;
+}
+
 // a1: one point of the AoS input.  Loaded one tile ahead of its use (software prefetch): under a saturated
 // write stream the read latency is several microseconds, and nothing else in a warp's tile depends on memory.
-template <typename TI>
+template <typename TI, bool ANGULAR = false>
 struct RawPoint {
     TI x, y, z;
-    __device__ __forceinline__ void load(const TI* __restrict__ xyz, int64_t i) {
-        const TI* p = xyz + 3 * i;
-        x = __ldg(p); y = __ldg(p + 1); z = __ldg(p + 2);
+    // coords: Cartesian / normalized Cartesian points are [n][3]; angular points are [n][2] = (theta, phi).
+    // ANGULAR is a compile-time switch: the fp64 sincos slow path is a real function call, and kernels that contain
+    // it get a much larger register allocation, so the Cartesian kernels must not.
+    __device__ __forceinline__ void load(const TI* __restrict__ in, int64_t i) {
+        if constexpr (ANGULAR) {
+            const TI* p = in + 2 * i;
+            x = __ldg(p); y = __ldg(p + 1); z = TI(0);
+        } else {
+            const TI* p = in + 3 * i;
+            x = __ldg(p); y = __ldg(p + 1); z = __ldg(p + 2);
+        }
     }
-    __device__ __forceinline__ UnitVec unit() const { return normalize((double)x, (double)y, (double)z); }
+    __device__ __forceinline__ UnitVec unit(int coords) const {
+        if constexpr (ANGULAR) return from_angles((double)x, (double)y);
+        if (coords == SH_COORDS_NORMALIZED) return as_given((double)x, (double)y, (double)z);
+        return normalize((double)x, (double)y, (double)z);
+    }
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -100,8 +155,8 @@ struct Azim {
     }
 };
 
-template <int LMAX, typename T, class Sink>
-__device__ __forceinline__ void eval_real(T x, T y, T z, bool origin, Sink& sink) {
+template <int LMAX, typename T, class O, class Sink>
+__device__ __forceinline__ void eval_real(T x, T y, T z, O origin, Sink& sink) {
     const Azim<LMAX, T> az(x, y);
     static_for<0, LMAX + 1>([&](auto lc) {
         constexpr int L = decltype(lc)::value;
@@ -112,7 +167,7 @@ __device__ __forceinline__ void eval_real(T x, T y, T z, bool origin, Sink& sink
             q[M] = T(A) * shgen::Polar<L, M, T>::eval(z);
         });
         // r = 0: x = y = z = 0 zeroes everything except the even-l, m = 0 polynomials (P_l(0) != 0)
-        if constexpr (L > 0 && L % 2 == 0) { if (origin) q[0] = T(0); }
+        if constexpr (L > 0 && L % 2 == 0) q[0] = zero_where(origin, q[0]);
         static_for<0, L>([&](auto jc) {
             constexpr int M = L - decltype(jc)::value;
             sink.template put1<L * (L + 1) - M>(q[M] * az.S[M]);
@@ -136,7 +191,7 @@ __device__ __forceinline__ void complex_block(const Azim<LMAX, T>& az, T z, bool
         a[M] = u * az.C[M];
         b[M] = u * az.S[M];
     });
-    if constexpr (L > 0 && L % 2 == 0) { if (origin) a[0] = T(0); }
+    if constexpr (L > 0 && L % 2 == 0) a[0] = zero_where(origin, a[0]);
 }
 
 template <int LMAX, typename T, class Sink>
@@ -204,6 +259,13 @@ __device__ __forceinline__ void evaluate(const UnitVec& u, Sink& sink) {
     else eval_spinor<LMAX, T>(x, y, z, u.origin, sink);
 }
 
+// two points per thread (fp32 variant): fp64 normalization of each, rounded once, then packed-fp32 polynomials
+template <int LMAX, class Sink>
+__device__ __forceinline__ void evaluate_pair(const UnitVec& u0, const UnitVec& u1, Sink& sink) {
+    const f2 x((float)u0.x, (float)u1.x), y((float)u0.y, (float)u1.y), z((float)u0.z, (float)u1.z);
+    eval_real<LMAX, f2>(x, y, z, Origin2{u0.origin, u1.origin}, sink);
+}
+
 // ------------------------------------------------------------------------------------------------
 // a8, SoA: element e of point i lives at out[(e*n + i) * ES .. +ES).  A warp writes 32*ES contiguous scalars
 // per element; streaming (evict-first) stores since nothing is re-read.  VEC = widest store in bytes the
@@ -231,14 +293,14 @@ struct SoASink {
     template <int L> __device__ __forceinline__ void end_l() {}
 };
 
-template <int KIND, int LMAX, typename T, typename TI, int VEC>
-__global__ void __launch_bounds__(256) sh_soa_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out, int tiles_per_cta) {
+template <int KIND, int LMAX, typename T, typename TI, int VEC, bool ANGULAR>
+__global__ void __launch_bounds__(256) sh_soa_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out, int tiles_per_cta, int coords) {
     constexpr int ES = elem_scalars(KIND);
     const int64_t ntiles = (n + 255) >> 8;
     int64_t t = (int64_t)blockIdx.x * tiles_per_cta;
     const int64_t tend = (t + tiles_per_cta < ntiles) ? t + tiles_per_cta : ntiles;
     int64_t i = (t << 8) + threadIdx.x;
-    RawPoint<TI> cur, nxt;
+    RawPoint<TI, ANGULAR> cur, nxt;
     bool have = i < n;
     if (have) cur.load(xyz, i);
     for (; t < tend; ++t, i += 256) {
@@ -246,9 +308,45 @@ __global__ void __launch_bounds__(256) sh_soa_kernel(const TI* __restrict__ xyz,
         if (have_next) nxt.load(xyz, i + 256);
         if (have) {
             SoASink<T, VEC> sink{out + i * ES, n * ES};
-            evaluate<KIND, LMAX, T>(cur.unit(), sink);
+            evaluate<KIND, LMAX, T>(cur.unit(coords), sink);
         }
         cur = nxt;
+        have = have_next;
+    }
+}
+
+// fp32 SoA, two ADJACENT points (2j, 2j+1) per thread: 8-byte stores (a warp store covers 256 B of a plane),
+// half the store and address instructions per point, packed-fp32 arithmetic.  Needs even n and 8-byte aligned out.
+struct SoAPairSink {
+    float* p;         // out + 2j
+    int64_t stride;   // n
+    template <int K> __device__ __forceinline__ void put1(f2 v) { __stcs(reinterpret_cast<float2*>(p + K * stride), v.v); }
+    template <int L> __device__ __forceinline__ void end_l() {}
+};
+
+template <int LMAX>
+__global__ void __launch_bounds__(256) sh_soa_pair_kernel(const float* __restrict__ xyz, int64_t n, float* __restrict__ out, int tiles_per_cta, int coords) {
+    const int64_t npairs = n >> 1;
+    const int64_t ntiles = (npairs + 255) >> 8;
+    int64_t t = (int64_t)blockIdx.x * tiles_per_cta;
+    const int64_t tend = (t + tiles_per_cta < ntiles) ? t + tiles_per_cta : ntiles;
+    int64_t j = (t << 8) + threadIdx.x;
+    auto load6 = [&](int64_t jj, float2& a, float2& b, float2& c) {
+        const float2* q = reinterpret_cast<const float2*>(xyz + 6 * jj);   // 24 B per pair: three 8-byte loads
+        a = __ldg(q); b = __ldg(q + 1); c = __ldg(q + 2);
+    };
+    float2 ca, cb, cc, na, nb, nc;
+    bool have = j < npairs;
+    if (have) load6(j, ca, cb, cc);
+    for (; t < tend; ++t, j += 256) {
+        const bool have_next = (t + 1 < tend) && (j + 256 < npairs);
+        if (have_next) load6(j + 256, na, nb, nc);
+        if (have) {
+            SoAPairSink sink{out + 2 * j, n};
+            if (coords == SH_COORDS_CARTESIAN) evaluate_pair<LMAX>(normalize(ca.x, ca.y, cb.x), normalize(cb.y, cc.x, cc.y), sink);
+            else evaluate_pair<LMAX>(as_given(ca.x, ca.y, cb.x), as_given(cb.y, cc.x, cc.y), sink);
+        }
+        ca = na; cb = nb; cc = nc;
         have = have_next;
     }
 }
@@ -394,8 +492,8 @@ struct RowSink {
     }
 };
 
-template <int KIND, int LMAX, typename T, typename TI, int CAP, int MODE, int WARPS>
-__global__ void __launch_bounds__(WARPS * 32) sh_aos_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out, int tiles_per_warp) {
+template <int KIND, int LMAX, typename T, typename TI, int CAP, int MODE, int WARPS, bool ANGULAR>
+__global__ void __launch_bounds__(WARPS * 32) sh_aos_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out, int tiles_per_warp, int coords) {
     using Sink = RowSink<KIND, LMAX, T, CAP, MODE>;
     static_assert(Sink::Seg::valid(), "CAP too small for one l-block group");
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -410,7 +508,7 @@ __global__ void __launch_bounds__(WARPS * 32) sh_aos_kernel(const TI* __restrict
         const int64_t i = (tt << 5) + lane;
         return (MODE == MODE_PLAIN && i >= n) ? n - 1 : i;
     };
-    RawPoint<TI> cur, nxt;
+    RawPoint<TI, ANGULAR> cur, nxt;
     bool have = t < tend && point_of(t) < n;
     if (have) cur.load(xyz, point_of(t));
     for (; t < tend; ++t) {
@@ -428,7 +526,7 @@ __global__ void __launch_bounds__(WARPS * 32) sh_aos_kernel(const TI* __restrict
             sink.lane = lane;
             sink.i = point_of(t);
             sink.wait_reads();   // bulk mode: the previous tile's copy has finished reading this lane's row
-            evaluate<KIND, LMAX, T>(cur.unit(), sink);
+            evaluate<KIND, LMAX, T>(cur.unit(coords), sink);
         }
         cur = nxt;
         have = have_next;
@@ -466,8 +564,8 @@ int tuned(int knob, int dflt) {
     return v > 0 ? v : dflt;
 }
 
-template <int KIND, int LMAX, typename T, typename TI, int VEC>
-int launch_soa(const TI* xyz, int64_t n, T* out, cudaStream_t st) {
+template <int KIND, int LMAX, typename T, typename TI, int VEC, bool ANGULAR = false>
+int launch_soa(const TI* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
     const int64_t tiles = (n + 255) / 256;
     // a few consecutive 256-point tiles per CTA so that the next tile's input load overlaps this tile's stores,
     // while the grid stays many waves deep (the hardware CTA scheduler balances the SMs)
@@ -475,7 +573,7 @@ int launch_soa(const TI* xyz, int64_t n, T* out, cudaStream_t st) {
     while (tpc > 1 && tiles / tpc < (int64_t)sm_count() * 16) tpc >>= 1;
     const int64_t blocks = (tiles + tpc - 1) / tpc;
     if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
-    sh_soa_kernel<KIND, LMAX, T, TI, VEC><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, out, tpc);
+    sh_soa_kernel<KIND, LMAX, T, TI, VEC, ANGULAR><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, out, tpc, coords);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? SH_OK : cuda_fail(e);
@@ -488,14 +586,14 @@ constexpr int aos_cap() {
     return KIND == KIND_SPINOR ? (200 > 8 * (2 * LMAX + 1) ? 200 : 8 * (2 * LMAX + 1)) : scalars_per_point(KIND, LMAX);
 }
 
-template <int KIND, int LMAX, typename T, typename TI, int MODE>
-int launch_aos(const TI* xyz, int64_t n, T* out, cudaStream_t st) {
+template <int KIND, int LMAX, typename T, typename TI, int MODE, bool ANGULAR = false>
+int launch_aos(const TI* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
     constexpr int CAP = aos_cap<KIND, LMAX>();
     constexpr int WARPS = 4;
     using Sink = RowSink<KIND, LMAX, T, CAP, MODE>;
     constexpr size_t smem = (size_t)WARPS * 32 * Sink::PITCH * sizeof(T);
     static_assert(smem <= 227 * 1024, "staging tile exceeds shared memory");
-    auto kern = sh_aos_kernel<KIND, LMAX, T, TI, CAP, MODE, WARPS>;
+    auto kern = sh_aos_kernel<KIND, LMAX, T, TI, CAP, MODE, WARPS, ANGULAR>;
     static int ctas_per_sm = 0;   // idempotent cache of a pure function of the kernel
     if (!ctas_per_sm) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -512,7 +610,20 @@ int launch_aos(const TI* xyz, int64_t n, T* out, cudaStream_t st) {
     while (tpw > 1 && ntiles / ((int64_t)WARPS * tpw) < (int64_t)sm_count() * ctas_per_sm * 4) tpw >>= 1;
     const int64_t blocks = (ntiles + (int64_t)WARPS * tpw - 1) / ((int64_t)WARPS * tpw);
     if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
-    kern<<<(unsigned)blocks, WARPS * 32, smem, st>>>(xyz, n, out, tpw);
+    kern<<<(unsigned)blocks, WARPS * 32, smem, st>>>(xyz, n, out, tpw, coords);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? SH_OK : cuda_fail(e);
+}
+
+template <int LMAX>
+int launch_soa_pair(const float* xyz, int64_t n, float* out, int coords, cudaStream_t st) {
+    const int64_t tiles = ((n >> 1) + 255) / 256;
+    int tpc = tuned(SH_TUNE_SOA_TILES_PER_CTA, 2);
+    while (tpc > 1 && tiles / tpc < (int64_t)sm_count() * 16) tpc >>= 1;
+    const int64_t blocks = (tiles + tpc - 1) / tpc;
+    if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
+    sh_soa_pair_kernel<LMAX><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, out, tpc, coords);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? SH_OK : cuda_fail(e);
@@ -521,43 +632,56 @@ int launch_aos(const TI* xyz, int64_t n, T* out, cudaStream_t st) {
 inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
 template <int KIND, int LMAX, typename T, typename TI>
-int dispatch_lmax(const TI* xyz, int64_t n, T* out, int layout, int path, cudaStream_t st) {
+int dispatch_lmax(const TI* xyz, int64_t n, T* out, int layout, int path, int coords, cudaStream_t st) {
     constexpr int SP = scalars_per_point(KIND, LMAX);
+    constexpr bool F32 = std::is_same<T, float>::value && KIND == KIND_REAL;
+    if (coords == SH_COORDS_ANGULAR) {
+        // angular front end: trigonometry dominates; it is served by the generic store paths only (scalar SoA stores,
+        // AoS staging + coalesced copy-out), which are valid for every alignment
+        if (path == SH_STORE_BULK) return SH_ERR_ALIGNMENT;
+        if (layout == SH_LAYOUT_SOA) return launch_soa<KIND, LMAX, T, TI, 8, true>(xyz, n, out, coords, st);
+        return launch_aos<KIND, LMAX, T, TI, MODE_PLAIN, true>(xyz, n, out, coords, st);
+    }
     if (layout == SH_LAYOUT_SOA) {
         if (path == SH_STORE_BULK) return SH_ERR_ALIGNMENT;   // bulk path is AoS only
         constexpr int ES = elem_scalars(KIND);
+        if constexpr (F32) {
+            // two adjacent points per thread (packed fp32, 8-byte stores) when every plane keeps 8-byte alignment
+            if (n >= 2 && n % 2 == 0 && aligned(out, 8) && aligned(xyz, 8) && path != SH_STORE_DIRECT)
+                return launch_soa_pair<LMAX>(reinterpret_cast<const float*>(xyz), n, reinterpret_cast<float*>(out), coords, st);
+        }
         // plane e starts at out + e*n*ES scalars: vector stores need that to stay aligned for every e
         const size_t plane_bytes = (size_t)n * ES * sizeof(T);
         if constexpr (ES * sizeof(T) >= 32) {
-            if (aligned(out, 32) && plane_bytes % 32 == 0) return launch_soa<KIND, LMAX, T, TI, 32>(xyz, n, out, st);
+            if (aligned(out, 32) && plane_bytes % 32 == 0) return launch_soa<KIND, LMAX, T, TI, 32>(xyz, n, out, coords, st);
         }
         if constexpr (ES * sizeof(T) >= 16) {
-            if (aligned(out, 16) && plane_bytes % 16 == 0) return launch_soa<KIND, LMAX, T, TI, 16>(xyz, n, out, st);
+            if (aligned(out, 16) && plane_bytes % 16 == 0) return launch_soa<KIND, LMAX, T, TI, 16>(xyz, n, out, coords, st);
         }
-        return launch_soa<KIND, LMAX, T, TI, 8>(xyz, n, out, st);
+        return launch_soa<KIND, LMAX, T, TI, 8>(xyz, n, out, coords, st);
     }
     const bool bulk_ok = aligned(out, 16) && (SP * sizeof(T)) % 16 == 0;
     if (path == SH_STORE_BULK && !bulk_ok) return SH_ERR_ALIGNMENT;
     if constexpr ((SP * sizeof(T)) % 16 == 0) {
-        if (bulk_ok && path != SH_STORE_DIRECT) return launch_aos<KIND, LMAX, T, TI, MODE_ROWBULK>(xyz, n, out, st);
+        if (bulk_ok && path != SH_STORE_DIRECT) return launch_aos<KIND, LMAX, T, TI, MODE_ROWBULK>(xyz, n, out, coords, st);
     }
-    return launch_aos<KIND, LMAX, T, TI, MODE_PLAIN>(xyz, n, out, st);
+    return launch_aos<KIND, LMAX, T, TI, MODE_PLAIN>(xyz, n, out, coords, st);
 }
 
 template <int KIND, typename T, typename TI>
 int run_device(const TI* xyz, int64_t n, int lmax, T* out, int layout_bits, void* stream) {
     if (n < 0) return SH_ERR_COUNT;
     if (lmax < 0 || lmax > shgen::LMAX_CAP) return SH_ERR_LMAX;
-    const int layout = layout_bits & 0xff, path = layout_bits & 0xff00;
-    if ((layout_bits & ~0xffff) || (layout != SH_LAYOUT_AOS && layout != SH_LAYOUT_SOA) ||
-        (path != SH_STORE_AUTO && path != SH_STORE_DIRECT && path != SH_STORE_BULK))
+    const int layout = layout_bits & 0xff, path = layout_bits & 0xff00, coords = layout_bits & 0x30000;
+    if ((layout_bits & ~0x3ffff) || (layout != SH_LAYOUT_AOS && layout != SH_LAYOUT_SOA) ||
+        (path != SH_STORE_AUTO && path != SH_STORE_DIRECT && path != SH_STORE_BULK) || coords == 0x30000)
         return SH_ERR_LAYOUT;
     if (n == 0) return SH_OK;
     if (!xyz || !out) return SH_ERR_NULL;
     if (!aligned(out, sizeof(T)) || !aligned(xyz, sizeof(TI))) return SH_ERR_ALIGNMENT;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     switch (lmax) {
-#define SH_CASE(L) case L: return dispatch_lmax<KIND, L, T, TI>(xyz, n, out, layout, path, st);
+#define SH_CASE(L) case L: return dispatch_lmax<KIND, L, T, TI>(xyz, n, out, layout, path, coords, st);
 #ifndef SHB200_DEV_ONLY_LMAX9   /* development builds may compile the lmax = 9 kernels only */
         SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(3) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8)
 #endif
@@ -572,10 +696,11 @@ template <int KIND, typename T, typename TI>
 int run_host(const TI* xyz, int64_t n, int lmax, T* out, int layout_bits) {
     if (n < 0) return SH_ERR_COUNT;
     if (lmax < 0 || lmax > shgen::LMAX_CAP) return SH_ERR_LMAX;
-    const int layout = layout_bits & 0xff;
-    if (layout != SH_LAYOUT_AOS && layout != SH_LAYOUT_SOA) return SH_ERR_LAYOUT;
+    const int layout = layout_bits & 0xff, coords = layout_bits & 0x30000;
+    if ((layout_bits & ~0x3ffff) || (layout != SH_LAYOUT_AOS && layout != SH_LAYOUT_SOA) || coords == 0x30000) return SH_ERR_LAYOUT;
     if (n == 0) return SH_OK;
     if (!xyz || !out) return SH_ERR_NULL;
+    const int64_t w = coords == SH_COORDS_ANGULAR ? 2 : 3;   // input scalars per point
     const int64_t sp = (int64_t)elem_scalars(KIND) * elems_per_point(KIND, lmax);   // scalars per point
     const int64_t es = elem_scalars(KIND), ne = sp / es;
     // chunk: ~256 MiB of output per buffer, a multiple of 256 points, at least 256
@@ -591,12 +716,12 @@ int run_host(const TI* xyz, int64_t n, int lmax, T* out, int layout_bits) {
     const int nbuf = n > chunk ? 2 : 1;
     for (int b = 0; b < nbuf && rc == SH_OK; ++b) {
         check(cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking)) &&
-            check(cudaMalloc(&dxyz[b], (size_t)chunk * 3 * sizeof(TI))) && check(cudaMalloc(&dout[b], (size_t)chunk * sp * sizeof(T)));
+            check(cudaMalloc(&dxyz[b], (size_t)chunk * w * sizeof(TI))) && check(cudaMalloc(&dout[b], (size_t)chunk * sp * sizeof(T)));
     }
     for (int64_t c0 = 0, it = 0; c0 < n && rc == SH_OK; c0 += chunk, ++it) {
         const int b = (int)(it % nbuf);
         const int64_t m = (n - c0) < chunk ? (n - c0) : chunk;
-        if (!check(cudaMemcpyAsync(dxyz[b], xyz + 3 * c0, (size_t)m * 3 * sizeof(TI), cudaMemcpyHostToDevice, st[b]))) break;
+        if (!check(cudaMemcpyAsync(dxyz[b], xyz + w * c0, (size_t)m * w * sizeof(TI), cudaMemcpyHostToDevice, st[b]))) break;
         int r = run_device<KIND, T, TI>(dxyz[b], m, lmax, dout[b], layout_bits, st[b]);
         if (r != SH_OK) { rc = r; break; }
         if (layout == SH_LAYOUT_AOS) {

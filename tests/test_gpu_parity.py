@@ -23,7 +23,7 @@ def sh():
     return pkg
 
 
-def gpu_eval(sh, kind, xyz, lmax, layout, store="auto", misalign=0):
+def gpu_eval(sh, kind, xyz, lmax, layout, store="auto", misalign=0, coords="cartesian"):
     """Run the CUDA path; returns a numpy array in the oracle's AoS shape."""
     import torch
 
@@ -35,7 +35,7 @@ def gpu_eval(sh, kind, xyz, lmax, layout, store="auto", misalign=0):
     backing = torch.full((numel + 8,), float("nan"), dtype=dt, device="cuda")
     out = backing[misalign : misalign + numel]
     fn = getattr(sh, "sh_" + kind)
-    fn(x, lmax, out=out, layout=layout, store=store)
+    fn(x, lmax, out=out, layout=layout, store=store, coords=coords)
     torch.cuda.synchronize()
     # guard elements around `out` untouched
     assert torch.isnan(backing[:misalign]).all() and torch.isnan(backing[misalign + numel :]).all()
@@ -162,6 +162,70 @@ def test_near_pole_points(sh, oracle_mod):
         assert max_err(got, oracle_eval(oracle_mod, kind, pts, 9)) <= TOL64
 
 
+def test_fp32_pair_and_scalar_paths(sh, oracle_mod, cube_points):
+    """fp32 SoA: even n and 8-byte aligned out -> two-points-per-thread packed-fp32 kernel; otherwise scalar kernel."""
+    x32 = cube_points.astype(np.float32)
+    for n in (10008, 10007, 3, 2, 1):
+        for mis in (0, 1):
+            for store in ("auto", "direct"):
+                got = gpu_eval(sh, "real_f32", x32[:n], 9, "soa", store, misalign=mis)
+                want = oracle_mod.real(x32[:n].astype(np.float64), 9)
+                assert max_err(got.astype(np.float64), want) <= TOL32, (n, mis, store)
+
+
+# ----------------------------------------------------------------------------- front ends (P:69)
+@pytest.mark.parametrize("kind", ["real", "complex", "spinor", "real_f32"])
+@pytest.mark.parametrize("layout", ["soa", "aos"])
+def test_normalized_and_angular_front_ends(sh, oracle_mod, kind, layout):
+    rng = np.random.default_rng(31)
+    g = rng.standard_normal((5003, 3))
+    unit = g / np.linalg.norm(g, axis=1)[:, None]
+    unit[:3] = [[0, 0, 1.0], [0, 0, -1.0], [1.0, 0, 0]]
+    unit[3] = 0.0  # zero vector: r = 0 convention (include/shb200.h)
+    theta = np.arccos(np.clip(unit[4:, 2], -1, 1))
+    phi = np.arctan2(unit[4:, 1], unit[4:, 0])
+    tp = np.stack([theta, phi], axis=1)
+    tp[:2] = [[0.0, 0.3], [np.pi, -2.0]]  # poles given as angles
+    tol = TOL32 if kind == "real_f32" else TOL64
+    if kind == "real_f32":
+        unit, tp = unit.astype(np.float32), tp.astype(np.float32)
+    for lmax in (0, 1, 4, 9):
+        got = gpu_eval(sh, kind, unit, lmax, layout, coords="normalized")
+        want = oracle_eval(oracle_mod, kind, unit.astype(np.float64), lmax)
+        assert max_err(got.astype(np.float64), want) <= tol, ("normalized", lmax)
+        got = gpu_eval(sh, kind, tp, lmax, layout, coords="angular")
+        k = (lmax + 1) ** 2
+        tp64 = tp.astype(np.float64)
+        if kind in ("real", "real_f32"):
+            want = oracle_mod.real_angular(tp64, lmax)
+        elif kind == "complex":
+            want = oracle_mod.complex_angular(tp64, lmax).view(np.float64).reshape(len(tp), k, 2)
+        else:
+            want = oracle_mod.spinor_angular(tp64, lmax).view(np.float64).reshape(len(tp), 2 * k, 4)
+        assert max_err(got.astype(np.float64), want) <= tol, ("angular", lmax)
+
+
+def test_paper_tables_through_the_angular_front_end(sh):
+    """The paper's own reference values (Appendix D, Tables II/III) against the CUDA path directly:
+    the printed (theta, phi) go through SH_COORDS_ANGULAR, no oracle involved."""
+    import os
+
+    golden = os.path.join(os.path.dirname(__file__), "golden", "paper_tables_II_III.txt")
+    pts = {"II": (2.12160245947564796, -1.82732370250979703), "III": (1.69050041976591414, 0.758228122208986166)}
+    tp = np.array([pts["II"], pts["III"]])
+    for layout in ("soa", "aos"):
+        got = gpu_eval(sh, "real", tp, 9, layout, coords="angular")
+        count = 0
+        for line in open(golden):
+            if line.startswith("#") or not line.strip():
+                continue
+            t, l, m, v, _ = line.split()
+            row = 0 if t == "II" else 1
+            assert abs(got[row, int(l) * (int(l) + 1) + int(m)] - float(v)) <= 2e-15, (t, l, m)
+            count += 1
+        assert count == 122
+
+
 # ----------------------------------------------------------------------------- config 2
 def test_config2_projector_grid(sh, oracle_mod):
     from paper_2510_05282_b200 import inputs
@@ -275,6 +339,12 @@ def test_config5_real_f32_variant(sh, oracle_mod, layout):
 def test_host_entry_points(sh, oracle_mod, kind, lmax, n, layout):
     rng = np.random.default_rng(77)
     pts = rng.uniform(-3, 3, (n, 3))
+    if kind == "spinor":  # also the angular front end through the host pipeline
+        tp = np.stack([rng.uniform(0, np.pi, n), rng.uniform(-np.pi, np.pi, n)], axis=1)
+        got = sh.host_call(kind, tp, lmax, layout=layout, coords="angular")
+        got = np.moveaxis(got, 0, 1) if layout == "soa" else got
+        want = oracle_mod.spinor_angular(tp, lmax).view(np.float64).reshape(n, 2 * (lmax + 1) ** 2, 4)
+        assert max_err(np.asarray(got).reshape(want.shape), want) <= TOL64
     if kind == "real_f32":
         pts = pts.astype(np.float32)
     got = sh.host_call(kind, pts, lmax, layout=layout)  # n = 400k at lmax 9: two pipeline chunks

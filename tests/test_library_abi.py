@@ -58,6 +58,8 @@ def test_argument_validation_without_gpu(lib):
         assert fn(p, 4, -1, p, 1, None) == -3
         assert fn(p, 4, 3, p, 2, None) == -4             # SH_ERR_LAYOUT
         assert fn(p, 4, 3, p, 0 | (3 << 8), None) == -4
+        assert fn(p, 4, 3, p, 0 | (3 << 16), None) == -4  # unknown front end
+        assert fn(p, 4, 3, p, 1 | (1 << 18), None) == -4
         assert fn(None, 4, 3, p, 0, None) == -1          # SH_ERR_NULL
         assert fn(p, 4, 3, None, 1, None) == -1
         assert fn(None, 0, 3, None, 0, None) == 0        # n = 0: successful no-op
