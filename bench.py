@@ -185,6 +185,19 @@ def extra_configs(sh, dev):
         return a.elapsed_time(b) / reps
 
     res = {}
+    # the paper's three front ends (Table I) on the headline workload, SoA
+    grid = inputs.config3_full_grid()
+    rr = np.linalg.norm(grid, axis=1)
+    rr[rr == 0] = 1.0
+    unit = np.ascontiguousarray(grid / rr[:, None])
+    ang = np.ascontiguousarray(np.stack([np.arccos(np.clip(unit[:, 2], -1, 1)), np.arctan2(unit[:, 1], unit[:, 0])], axis=1))
+    out = torch.empty((K, len(grid)), dtype=torch.float64, device=dev)
+    for coords, arr in (("cartesian", grid), ("normalized", unit), ("angular", ang)):
+        x = torch.from_numpy(arr).to(dev)
+        ms = timed(lambda: sh.sh_real(x, LMAX, out=out, layout="soa", coords=coords), 20)
+        res[f"config3 real l9 SoA front end {coords}"] = {"ms": ms, "write_GBps": len(grid) * K * 8 / ms / 1e6, "G_values_per_s": len(grid) * K / ms / 1e6}
+        del x
+    del out
     cases = [
         ("config1 real l4 SoA N=10008", "real", inputs.config1_cube(), 4, ["soa"], 50),
         ("config2 real l3 SoA N=113102", "real", inputs.config2_projector_grid(), 3, ["soa"], 50),
