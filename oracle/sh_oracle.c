@@ -39,9 +39,9 @@
  *           of 2l entries, then j = l+1/2 block of 2l+2 entries; m_j ascending)
  *
  * Parity pins: see tests/test_oracle_pins.py (Tables II/III of the paper, Appendix C formulas,
- * l <= 2 closed forms, Unsoeld sums, quadrature orthonormality, symmetries, scipy's sph_harm_y).
- * Spinor values beyond orthonormality, the sum rule and the l = 0, 1 hand cases: parity unpinned
- * (the paper prints no spinor values).
+ * l <= 2 closed forms, Unsoeld sums, quadrature orthonormality, symmetries, scipy's sph_harm_y,
+ * mpmath's spherharm).  The paper prints no spinor values: the spinor weights and signs are pinned
+ * against sympy's Clebsch-Gordan coefficients, plus orthonormality, the sum rule and hand cases.
  */
 #include <math.h>
 #include <stdint.h>

@@ -374,3 +374,32 @@ def test_bad_arguments(oracle_mod):
     with pytest.raises(ValueError):
         oracle_mod.real(np.zeros((1, 3)), -1)
     assert oracle_mod.real(np.zeros((0, 3)), 3).shape == (0, 16)
+
+
+def test_spinor_weights_against_sympy_clebsch_gordan(oracle_mod):
+    """Eq. 7 is the coupling of Y_l^{m_j -+ 1/2} with the spin-1/2 basis states: its weights must be the
+    Clebsch-Gordan coefficients <l m_l 1/2 m_s | j m_j> (Condon-Shortley convention).  sympy's CG is an independent
+    library routine; with the separately pinned Y_l^m this pins every spinor component, signs included."""
+    from sympy import Rational
+    from sympy.physics.quantum.cg import CG
+
+    pts = unit_vectors(40, 25) * 1.7
+    Y = oracle_mod.complex_(pts, 9)
+    S = oracle_mod.spinor(pts, 9)
+    half = Rational(1, 2)
+    worst = 0.0
+    for l in range(10):
+        for twoj in (2 * l - 1, 2 * l + 1):
+            if twoj < 1:
+                continue
+            j = Rational(twoj, 2)
+            for twomj in range(-twoj, twoj + 1, 2):
+                mj = Rational(twomj, 2)
+                m_up, m_dn = int(mj - half), int(mj + half)
+                cu = float(CG(l, m_up, half, half, j, mj).doit()) if abs(m_up) <= l else 0.0
+                cd = float(CG(l, m_dn, half, -half, j, mj).doit()) if abs(m_dn) <= l else 0.0
+                up = cu * Y[:, k_of(l, m_up)] if abs(m_up) <= l else 0 * Y[:, 0]
+                dn = cd * Y[:, k_of(l, m_dn)] if abs(m_dn) <= l else 0 * Y[:, 0]
+                s = S[:, oracle_mod.index_spinor(l, twoj, twomj)]
+                worst = max(worst, np.abs(s[:, 0] - up).max(), np.abs(s[:, 1] - dn).max())
+    assert worst <= 2e-16, worst
