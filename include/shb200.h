@@ -94,12 +94,15 @@ int sh_real_f32(const float* xyz, int64_t n, int lmax, float* out, int layout, v
 
 /* Host-buffer entry points: same results, `xyz` and `out` are HOST pointers (pinned memory gives full
  * PCIe speed; pageable memory works).  The call copies chunks host->device, runs the kernels and copies
- * device->host on internal streams with double buffering, and returns after `out` is complete.  It
- * allocates and frees its own device staging buffers (at most ~1 GiB). */
+ * device->host on two internal streams with double buffering, and returns after `out` is complete.  The
+ * staging buffers (640 MiB of device memory) and streams are created on the first host call and kept for
+ * later ones; sh_host_release() frees them.  Host calls are serialized among themselves (internal mutex). */
 int sh_real_host(const double* xyz, int64_t n, int lmax, double* out, int layout);
 int sh_complex_host(const double* xyz, int64_t n, int lmax, double* out, int layout);
 int sh_spinor_host(const double* xyz, int64_t n, int lmax, double* out, int layout);
 int sh_real_f32_host(const float* xyz, int64_t n, int lmax, float* out, int layout);
+/* Frees the staging buffers and streams of the host entry points (no-op if there are none). */
+void sh_host_release(void);
 
 /* Scalars (doubles for the fp64 calls, floats for sh_real_f32) written per point; -1 if lmax is out of range. */
 int64_t sh_real_count(int lmax);    /* K   */

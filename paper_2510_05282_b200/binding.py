@@ -66,6 +66,7 @@ def load() -> ctypes.CDLL:
         lib.sh_strerror.restype = ctypes.c_char_p
         lib.sh_last_cuda_error.restype = ctypes.c_char_p
         lib.sh_kernel_launch_count.restype = i64
+        lib.sh_host_release.restype = None
         _lib = lib
     return _lib
 

@@ -20,6 +20,7 @@
 #include <cfloat>
 #include <cstdint>
 #include <cstring>
+#include <mutex>
 #include <type_traits>
 
 #include "../../include/shb200.h"
@@ -691,7 +692,44 @@ int run_device(const TI* xyz, int64_t n, int lmax, T* out, int layout_bits, void
     return SH_ERR_LMAX;
 }
 
-// Host-buffer pipeline: chunks of points go host -> device -> kernel -> host on two streams (double buffering).
+// Host-buffer pipeline: chunks of points go host -> device -> kernel -> host on two streams (double buffering):
+// the device->host copy of chunk c overlaps the host->device copy and the kernel of chunk c+1.
+// The two staging slots (64 MiB input + 256 MiB output each) and their streams are created on first use and
+// kept for later calls (cudaMalloc/cudaFree per call cost milliseconds and cudaFree synchronizes the device);
+// sh_host_release() frees them.  One host call at a time uses the pool (mutex); device calls never touch it.
+struct HostPool {
+    std::mutex mu;
+    int device = -1;
+    cudaStream_t st[2] = {nullptr, nullptr};
+    void* din[2] = {nullptr, nullptr};
+    void* dout[2] = {nullptr, nullptr};
+    static constexpr size_t IN_CAP = (size_t)64 << 20, OUT_CAP = (size_t)256 << 20;
+    void release() {
+        for (int b = 0; b < 2; ++b) {
+            if (st[b]) cudaStreamDestroy(st[b]);
+            if (din[b]) cudaFree(din[b]);
+            if (dout[b]) cudaFree(dout[b]);
+            st[b] = nullptr; din[b] = nullptr; dout[b] = nullptr;
+        }
+        device = -1;
+    }
+    cudaError_t ensure() {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        if (device == dev && st[1] && dout[1]) return cudaSuccess;
+        release();
+        for (int b = 0; b < 2; ++b) {
+            if ((e = cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking)) != cudaSuccess) return e;
+            if ((e = cudaMalloc(&din[b], IN_CAP)) != cudaSuccess) return e;
+            if ((e = cudaMalloc(&dout[b], OUT_CAP)) != cudaSuccess) return e;
+        }
+        device = dev;
+        return cudaSuccess;
+    }
+};
+HostPool g_pool;
+
 template <int KIND, typename T, typename TI>
 int run_host(const TI* xyz, int64_t n, int lmax, T* out, int layout_bits) {
     if (n < 0) return SH_ERR_COUNT;
@@ -703,40 +741,35 @@ int run_host(const TI* xyz, int64_t n, int lmax, T* out, int layout_bits) {
     const int64_t w = coords == SH_COORDS_ANGULAR ? 2 : 3;   // input scalars per point
     const int64_t sp = (int64_t)elem_scalars(KIND) * elems_per_point(KIND, lmax);   // scalars per point
     const int64_t es = elem_scalars(KIND), ne = sp / es;
-    // chunk: ~256 MiB of output per buffer, a multiple of 256 points, at least 256
-    int64_t chunk = ((int64_t)256 << 20) / (sp * (int64_t)sizeof(T));
+    // chunk: what fits a staging slot, a multiple of 256 points
+    int64_t chunk = (int64_t)(HostPool::OUT_CAP / (size_t)(sp * (int64_t)sizeof(T)));
+    const int64_t chunk_in = (int64_t)(HostPool::IN_CAP / (size_t)(w * (int64_t)sizeof(TI)));
+    if (chunk > chunk_in) chunk = chunk_in;
     chunk = chunk / 256 * 256;
-    if (chunk < 256) chunk = 256;
     if (chunk > n) chunk = n;
-    cudaStream_t st[2] = {nullptr, nullptr};
-    TI* dxyz[2] = {nullptr, nullptr};
-    T* dout[2] = {nullptr, nullptr};
+    std::lock_guard<std::mutex> lock(g_pool.mu);
     int rc = SH_OK;
     auto check = [&](cudaError_t e) { if (e != cudaSuccess && rc == SH_OK) rc = cuda_fail(e); return e == cudaSuccess; };
-    const int nbuf = n > chunk ? 2 : 1;
-    for (int b = 0; b < nbuf && rc == SH_OK; ++b) {
-        check(cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking)) &&
-            check(cudaMalloc(&dxyz[b], (size_t)chunk * w * sizeof(TI))) && check(cudaMalloc(&dout[b], (size_t)chunk * sp * sizeof(T)));
-    }
+    if (!check(g_pool.ensure())) { g_pool.release(); return rc; }
     for (int64_t c0 = 0, it = 0; c0 < n && rc == SH_OK; c0 += chunk, ++it) {
-        const int b = (int)(it % nbuf);
+        const int b = (int)(it & 1);
+        cudaStream_t st = g_pool.st[b];
+        TI* dxyz = static_cast<TI*>(g_pool.din[b]);
+        T* dout = static_cast<T*>(g_pool.dout[b]);
         const int64_t m = (n - c0) < chunk ? (n - c0) : chunk;
-        if (!check(cudaMemcpyAsync(dxyz[b], xyz + w * c0, (size_t)m * w * sizeof(TI), cudaMemcpyHostToDevice, st[b]))) break;
-        int r = run_device<KIND, T, TI>(dxyz[b], m, lmax, dout[b], layout_bits, st[b]);
+        // stream order makes slot b safe to reuse: its previous device->host copy precedes this host->device copy
+        if (!check(cudaMemcpyAsync(dxyz, xyz + w * c0, (size_t)m * w * sizeof(TI), cudaMemcpyHostToDevice, st))) break;
+        int r = run_device<KIND, T, TI>(dxyz, m, lmax, dout, layout_bits, st);
         if (r != SH_OK) { rc = r; break; }
         if (layout == SH_LAYOUT_AOS) {
-            check(cudaMemcpyAsync(out + c0 * sp, dout[b], (size_t)m * sp * sizeof(T), cudaMemcpyDeviceToHost, st[b]));
+            check(cudaMemcpyAsync(out + c0 * sp, dout, (size_t)m * sp * sizeof(T), cudaMemcpyDeviceToHost, st));
         } else {
             // device chunk is [ne][m] elements; host array is [ne][n]: one strided 2-D copy
-            check(cudaMemcpy2DAsync(out + c0 * es, (size_t)n * es * sizeof(T), dout[b], (size_t)m * es * sizeof(T),
-                                    (size_t)m * es * sizeof(T), (size_t)ne, cudaMemcpyDeviceToHost, st[b]));
+            check(cudaMemcpy2DAsync(out + c0 * es, (size_t)n * es * sizeof(T), dout, (size_t)m * es * sizeof(T),
+                                    (size_t)m * es * sizeof(T), (size_t)ne, cudaMemcpyDeviceToHost, st));
         }
     }
-    for (int b = 0; b < nbuf; ++b) {
-        if (st[b]) { check(cudaStreamSynchronize(st[b])); cudaStreamDestroy(st[b]); }
-        if (dxyz[b]) cudaFree(dxyz[b]);
-        if (dout[b]) cudaFree(dout[b]);
-    }
+    for (int b = 0; b < 2; ++b) check(cudaStreamSynchronize(g_pool.st[b]));
     return rc;
 }
 
@@ -769,6 +802,11 @@ int sh_spinor_host(const double* xyz, int64_t n, int lmax, double* out, int layo
 }
 int sh_real_f32_host(const float* xyz, int64_t n, int lmax, float* out, int layout) {
     return run_host<KIND_REAL, float, float>(xyz, n, lmax, out, layout);
+}
+
+void sh_host_release(void) {
+    std::lock_guard<std::mutex> lock(g_pool.mu);
+    g_pool.release();
 }
 
 int64_t sh_real_count(int lmax) { return (lmax < 0 || lmax > 9) ? -1 : (int64_t)(lmax + 1) * (lmax + 1); }
