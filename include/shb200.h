@@ -57,7 +57,8 @@ enum {
 enum {
     SH_STORE_AUTO   = 0 << 8,
     SH_STORE_DIRECT = 1 << 8, /* per-thread st.global.cs; SoA: coalesced planes; AoS: smem transpose + coalesced stores */
-    SH_STORE_BULK   = 2 << 8  /* AoS only: per-point rows staged in shared memory, written by TMA bulk copies (cp.async.bulk) */
+    SH_STORE_BULK   = 2 << 8  /* AoS only, needs a 16-byte aligned out: rows staged in shared memory, written by TMA bulk copies
+                                 (cp.async.bulk): one copy per 32-point tile where the layout allows, else one per row */
 };
 
 /* Input front end, OR-ed into `layout` (bits 16-17).  Default: Cartesian.
@@ -120,7 +121,8 @@ int sh_index_spinor(int l, int twoj, int twomj);
 enum {
     SH_TUNE_SOA_TILES_PER_CTA = 0,  /* consecutive 256-point tiles one CTA of the SoA kernels processes */
     SH_TUNE_AOS_TILES_PER_WARP = 1, /* consecutive 32-point tiles one warp of the AoS kernels processes */
-    SH_TUNE_COUNT = 2
+    SH_TUNE_PREFETCH_WINDOW_POINTS = 2, /* points per burst of the L2 input prefetch (default 262144); 1 = prefetch off */
+    SH_TUNE_COUNT = 3
 };
 int sh_set_tuning(int knob, int value);
 

@@ -30,7 +30,7 @@
 namespace {
 
 constexpr int KIND_REAL = 0, KIND_COMPLEX = 1, KIND_SPINOR = 2;
-constexpr int MODE_PLAIN = 0, MODE_ROWBULK = 1;
+constexpr int MODE_PLAIN = 0, MODE_ROWBULK = 1, MODE_TILEBULK = 2;
 
 // ------------------------------------------------------------------------------------------------
 // compile-time loop
@@ -141,6 +141,32 @@ struct RawPoint {
         return normalize((double)x, (double)y, (double)z);
     }
 };
+
+// a1, second half: burst prefetch of the input into L2.  The 24 B/point of input are 3 % of the traffic, but read
+// requests sprinkled into a saturated write stream cost ~4x their share (each one turns DRAM channels around:
+// 241 -> 274 us on a store-only model of the lmax = 9 SoA kernel).  So reads are issued in bursts, far ahead of use:
+// the grid is cut into windows of `win_ctas` consecutive CTAs; the first `spread` CTAs of window w (they start at about
+// the same time on different SMs) prefetch the whole input of window w + 1 (window 0: of windows 0 and 1) into L2
+// with evict_last priority -- the streaming evict-first stores of the outputs then do not push it out before the
+// demand loads arrive (with normal priority they do: no gain measured).  A hint only: results never depend on it.
+struct InputPrefetch {
+    int win_ctas;   // 0 = off
+    int spread;
+};
+
+__device__ __forceinline__ void prefetch_input_window(const void* in, int64_t total_bytes, int64_t bytes_per_cta, InputPrefetch pf) {
+    if (pf.win_ctas <= 0) return;
+    const int w = blockIdx.x / pf.win_ctas, r = blockIdx.x - w * pf.win_ctas;
+    if (r >= pf.spread) return;
+    const int64_t wbytes = (int64_t)pf.win_ctas * bytes_per_cta;
+    int64_t lo = (int64_t)(w + 1) * wbytes;
+    const int64_t hi = lo + wbytes < total_bytes ? lo + wbytes : total_bytes;
+    if (w == 0) lo = 0;
+    const char* base = static_cast<const char*>(in);
+    const int64_t step = (int64_t)pf.spread * blockDim.x * 128;
+    for (int64_t o = lo + ((int64_t)r * blockDim.x + threadIdx.x) * 128; o < hi; o += step)
+        asm volatile("prefetch.global.L2::evict_last [%0];" ::"l"(base + o));
+}
 
 // ------------------------------------------------------------------------------------------------
 // a3-a7: evaluators.  Sink interface: put1<K>(v) real element K; put2<K>(re, im) complex element K;
@@ -295,8 +321,10 @@ struct SoASink {
 };
 
 template <int KIND, int LMAX, typename T, typename TI, int VEC, bool ANGULAR>
-__global__ void __launch_bounds__(256) sh_soa_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out, int tiles_per_cta, int coords) {
+__global__ void __launch_bounds__(256) sh_soa_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out, int tiles_per_cta, int coords, InputPrefetch pf) {
     constexpr int ES = elem_scalars(KIND);
+    constexpr int IN_BYTES = (ANGULAR ? 2 : 3) * sizeof(TI);
+    prefetch_input_window(xyz, n * IN_BYTES, (int64_t)tiles_per_cta * 256 * IN_BYTES, pf);
     const int64_t ntiles = (n + 255) >> 8;
     int64_t t = (int64_t)blockIdx.x * tiles_per_cta;
     const int64_t tend = (t + tiles_per_cta < ntiles) ? t + tiles_per_cta : ntiles;
@@ -326,7 +354,8 @@ struct SoAPairSink {
 };
 
 template <int LMAX>
-__global__ void __launch_bounds__(256) sh_soa_pair_kernel(const float* __restrict__ xyz, int64_t n, float* __restrict__ out, int tiles_per_cta, int coords) {
+__global__ void __launch_bounds__(256) sh_soa_pair_kernel(const float* __restrict__ xyz, int64_t n, float* __restrict__ out, int tiles_per_cta, int coords, InputPrefetch pf) {
+    prefetch_input_window(xyz, n * 12, (int64_t)tiles_per_cta * 512 * 12, pf);
     const int64_t npairs = n >> 1;
     const int64_t ntiles = (npairs + 255) >> 8;
     int64_t t = (int64_t)blockIdx.x * tiles_per_cta;
@@ -357,12 +386,17 @@ __global__ void __launch_bounds__(256) sh_soa_pair_kernel(const float* __restric
 // (or a segment of whole l-blocks of it, at most CAP scalars) in its own shared-memory row, then
 //   MODE_ROWBULK: the lane issues ONE TMA bulk copy (cp.async.bulk.global.shared::cta) for its segment;
 //                 needs 16-byte aligned global segments.  No warp-level synchronization at all.
+//   MODE_TILEBULK: whole rows are staged DENSELY (pitch = row), so the warp's 32-row tile is one contiguous span of
+//                 `out`; after a __syncwarp one lane issues ONE bulk copy for the whole tile (25.6 KB at lmax = 9).
+//                 One large TMA request per tile instead of 32 small ones: 7.4 vs 6.3-6.7 TB/s on a store-only model.
+//                 Dense rows cost 2-way bank conflicts on the 16-byte staging stores when the row is 32 (mod 128) bytes
+//                 (lmax = 9: 800 B); layouts where it would be worse (tile_bulk_ok) stay on MODE_ROWBULK.
 //   MODE_PLAIN:   the warp copies the staged tile out with coalesced streaming stores (any alignment).
 template <int KIND, int LMAX, int TSIZE, int CAP, int MODE>
 struct Segments {
     static constexpr int SP = scalars_per_point(KIND, LMAX);
     // a cut before block l is allowed where the row offset keeps the copy granularity (16 B for bulk)
-    static constexpr bool cut_ok(int l) { return l == LMAX + 1 || MODE == MODE_PLAIN || (cum_scalars(KIND, l) * TSIZE) % 16 == 0; }
+    static constexpr bool cut_ok(int l) { return l == LMAX + 1 || MODE == MODE_PLAIN || (MODE == MODE_ROWBULK && (cum_scalars(KIND, l) * TSIZE) % 16 == 0); }
     // greedy: the segment starting at block s ends before block seg_end(s)
     static constexpr int seg_end(int s) {
         int best = -1;
@@ -394,6 +428,7 @@ struct Segments {
     // row pitch in scalars: conflict-free staging stores.  bulk: 16-byte stores, odd number of 16-byte chunks;
     // plain: scalar stores, odd number of 8-byte (fp64) / 4-byte (fp32) words.
     static constexpr int pitch() {
+        if (MODE == MODE_TILEBULK) return SP;
         if (MODE == MODE_ROWBULK) {
             int chunks = (max_len() * TSIZE + 15) / 16;
             return (chunks | 1) * 16 / TSIZE;
@@ -410,6 +445,8 @@ struct RowSink {
     static constexpr int SP = Seg::SP;
     static constexpr int PITCH = Seg::pitch();
     static constexpr int VPC = 16 / sizeof(T);   // scalars per 16-byte chunk
+    // 16-byte staging stores: always in row-bulk mode (padded, aligned rows); in tile-bulk mode when dense rows keep 16-byte alignment
+    static constexpr bool VSTAGE = MODE == MODE_ROWBULK || (MODE == MODE_TILEBULK && (SP * sizeof(T)) % 16 == 0);
 
     T* row;          // this lane's staging row (shared memory)
     T* tile;         // the warp's staging tile (32 rows)
@@ -429,7 +466,7 @@ struct RowSink {
 
     template <int K> __device__ __forceinline__ void put1(T v) {
         constexpr int O = off<K, l_of_real<K>()>();
-        if constexpr (MODE == MODE_PLAIN) {
+        if constexpr (!VSTAGE) {
             row[O] = v;
         } else if constexpr (sizeof(T) == 8) {
             if constexpr (K % 2 == 0) hold[0] = v;
@@ -441,17 +478,31 @@ struct RowSink {
     }
     template <int K> __device__ __forceinline__ void put2(T re, T im) {
         constexpr int O = off<2 * K, l_of_real<K>()>();
-        if constexpr (MODE == MODE_PLAIN) { row[O] = re; row[O + 1] = im; }
+        if constexpr (!VSTAGE) { row[O] = re; row[O + 1] = im; }
         else st16(row + O, re, im);
     }
     template <int S> __device__ __forceinline__ void put4(T a, T b, T c, T d) {
         constexpr int O = off<4 * S, l_of_spinor<S>()>();
-        if constexpr (MODE == MODE_PLAIN) { row[O] = a; row[O + 1] = b; row[O + 2] = c; row[O + 3] = d; }
+        if constexpr (!VSTAGE) { row[O] = a; row[O + 1] = b; row[O + 2] = c; row[O + 3] = d; }
         else { st16(row + O, a, b); st16(row + O + 2, c, d); }
     }
 
     __device__ __forceinline__ void wait_reads() {
-        if constexpr (MODE == MODE_ROWBULK) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        if constexpr (MODE != MODE_PLAIN) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        if constexpr (MODE == MODE_TILEBULK) __syncwarp();   // lane 0 owns the tile's bulk group; nobody restages before it has been read
+    }
+
+    // coalesced copy-out of `rows` staged rows (tile-contiguous in `out` when whole rows are staged)
+    __device__ __forceinline__ void copy_out_whole_rows() {
+        T* g = gout + base * SP;
+        const int total = rows * SP;
+        int r = 0, c = lane;
+        while (c >= SP) { c -= SP; ++r; }
+        for (int e = lane; e < total; e += 32) {
+            __stcs(g + e, tile[r * PITCH + c]);
+            c += 32;
+            while (c >= SP) { c -= SP; ++r; }
+        }
     }
 
     template <int L> __device__ __forceinline__ void end_l() {
@@ -468,19 +519,27 @@ struct RowSink {
                              : "memory");
                 asm volatile("cp.async.bulk.commit_group;" ::: "memory");
                 if constexpr (L < LMAX) wait_reads();   // the row is reused by the next segment
+            } else if constexpr (MODE == MODE_TILEBULK) {
+                static_assert(LEN == SP && PITCH == SP, "tile-bulk mode stages whole dense rows");
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // every lane: its staging stores -> async proxy
+                __syncwarp();
+                const int bytes = rows * SP * (int)sizeof(T);
+                if (bytes % 16 == 0) {   // always for a full tile; a ragged last tile with an odd scalar count is copied by the warp
+                    if (lane == 0) {
+                        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gout + base * SP),
+                                     "r"(smem_u32(tile)), "r"(bytes)
+                                     : "memory");
+                        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                    }
+                } else {
+                    copy_out_whole_rows();
+                    __syncwarp();
+                }
             } else {
                 __syncwarp();
                 if constexpr (LEN == SP) {
                     // whole rows staged: the tile is one contiguous span of rows*SP scalars in `out`
-                    T* g = gout + base * SP;
-                    const int total = rows * SP;
-                    int r = 0, c = lane;
-                    while (c >= SP) { c -= SP; ++r; }
-                    for (int e = lane; e < total; e += 32) {
-                        __stcs(g + e, tile[r * PITCH + c]);
-                        c += 32;
-                        while (c >= SP) { c -= SP; ++r; }
-                    }
+                    copy_out_whole_rows();
                 } else {
                     for (int r = 0; r < rows; ++r) {
                         T* g = gout + (base + r) * SP + BEGIN;
@@ -494,8 +553,10 @@ struct RowSink {
 };
 
 template <int KIND, int LMAX, typename T, typename TI, int CAP, int MODE, int WARPS, bool ANGULAR>
-__global__ void __launch_bounds__(WARPS * 32) sh_aos_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out, int tiles_per_warp, int coords) {
+__global__ void __launch_bounds__(WARPS * 32) sh_aos_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out, int tiles_per_warp, int coords, InputPrefetch pf) {
     using Sink = RowSink<KIND, LMAX, T, CAP, MODE>;
+    constexpr int IN_BYTES = (ANGULAR ? 2 : 3) * sizeof(TI);
+    prefetch_input_window(xyz, n * IN_BYTES, (int64_t)tiles_per_warp * WARPS * 32 * IN_BYTES, pf);
     static_assert(Sink::Seg::valid(), "CAP too small for one l-block group");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -504,10 +565,10 @@ __global__ void __launch_bounds__(WARPS * 32) sh_aos_kernel(const TI* __restrict
     // warp w of CTA b owns tiles [(b*WARPS + w) * tiles_per_warp, +tiles_per_warp): a contiguous span of `out`
     int64_t t = ((int64_t)blockIdx.x * WARPS + warp) * tiles_per_warp;
     const int64_t tend = (t + tiles_per_warp < ntiles) ? t + tiles_per_warp : ntiles;
-    // plain mode: every lane takes part in the copy-out, so idle lanes of the last tile evaluate a clamped point
+    // plain / tile-bulk mode: every lane takes part in the warp-level copy-out, so idle lanes of the last tile evaluate a clamped point
     auto point_of = [&](int64_t tt) {
         const int64_t i = (tt << 5) + lane;
-        return (MODE == MODE_PLAIN && i >= n) ? n - 1 : i;
+        return (MODE != MODE_ROWBULK && i >= n) ? n - 1 : i;
     };
     RawPoint<TI, ANGULAR> cur, nxt;
     bool have = t < tend && point_of(t) < n;
@@ -532,7 +593,7 @@ __global__ void __launch_bounds__(WARPS * 32) sh_aos_kernel(const TI* __restrict
         cur = nxt;
         have = have_next;
     }
-    if constexpr (MODE == MODE_ROWBULK) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    if constexpr (MODE != MODE_PLAIN) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -565,16 +626,30 @@ int tuned(int knob, int dflt) {
     return v > 0 ? v : dflt;
 }
 
+// window plan of the burst input prefetch for a launch whose CTAs own `points_per_cta` consecutive points each
+InputPrefetch prefetch_plan(int64_t n, int64_t points_per_cta) {
+    const int64_t win_points = tuned(SH_TUNE_PREFETCH_WINDOW_POINTS, 1 << 18);   // 6 MiB of fp64 xyz per burst
+    InputPrefetch pf{0, 0};
+    if (win_points <= 1 || n <= win_points) return pf;   // knob value 1 = off; one window: the first wave reads it all anyway
+    int64_t win = win_points / points_per_cta;
+    if (win < 1) win = 1;
+    if (win > 0x3fffffff) return pf;
+    pf.win_ctas = (int)win;
+    pf.spread = win < sm_count() ? (int)win : sm_count();
+    return pf;
+}
+
 template <int KIND, int LMAX, typename T, typename TI, int VEC, bool ANGULAR = false>
 int launch_soa(const TI* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
     const int64_t tiles = (n + 255) / 256;
-    // a few consecutive 256-point tiles per CTA so that the next tile's input load overlaps this tile's stores,
-    // while the grid stays many waves deep (the hardware CTA scheduler balances the SMs)
-    int tpc = tuned(SH_TUNE_SOA_TILES_PER_CTA, 2);
+    // one 256-point tile per CTA: with the burst L2 prefetch the input load is an L2 hit, and a deep grid lets the
+    // hardware CTA scheduler balance the SMs (251 vs 256 / 258 us for 1 / 2 / 4 tiles on the 128^3 grid at lmax = 9).
+    // With more tiles per CTA the next tile's input is loaded before the current tile is evaluated.
+    int tpc = tuned(SH_TUNE_SOA_TILES_PER_CTA, 1);
     while (tpc > 1 && tiles / tpc < (int64_t)sm_count() * 16) tpc >>= 1;
     const int64_t blocks = (tiles + tpc - 1) / tpc;
     if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
-    sh_soa_kernel<KIND, LMAX, T, TI, VEC, ANGULAR><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, out, tpc, coords);
+    sh_soa_kernel<KIND, LMAX, T, TI, VEC, ANGULAR><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, out, tpc, coords, prefetch_plan(n, (int64_t)tpc * 256));
     g_launches.fetch_add(1, std::memory_order_relaxed);
     cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? SH_OK : cuda_fail(e);
@@ -585,6 +660,19 @@ int launch_soa(const TI* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
 template <int KIND, int LMAX>
 constexpr int aos_cap() {
     return KIND == KIND_SPINOR ? (200 > 8 * (2 * LMAX + 1) ? 200 : 8 * (2 * LMAX + 1)) : scalars_per_point(KIND, LMAX);
+}
+
+// tile-bulk mode: whole rows of a 32-point tile staged densely must fit (4 warps, 2 CTAs per SM), and the staging stores
+// must not conflict more than 2-way: 16-byte stores of a quarter warp land gcd(row_bytes/16, 8) deep; rows that are not
+// multiples of 16 B are staged with scalar stores, conflict-free because the row is then an odd number of words
+template <int KIND, int LMAX, typename T>
+constexpr bool tile_bulk_ok() {
+    constexpr int row_bytes = scalars_per_point(KIND, LMAX) * (int)sizeof(T);
+    if (KIND == KIND_SPINOR || 4 * 32 * row_bytes > 110 * 1024) return false;
+    if (row_bytes % 16 != 0) return true;
+    int chunks = row_bytes / 16, g = 8;
+    while (chunks % g) g >>= 1;
+    return g <= 2;
 }
 
 template <int KIND, int LMAX, typename T, typename TI, int MODE, bool ANGULAR = false>
@@ -605,13 +693,14 @@ int launch_aos(const TI* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
         ctas_per_sm = occ > 0 ? occ : 1;
     }
     const int64_t ntiles = (n + 31) / 32;
-    // a few consecutive tiles per warp (input prefetch across tiles, staging rows reused), many CTAs per SM over the
-    // run so that the hardware CTA scheduler evens out SM-to-SM speed differences
-    int tpw = tuned(SH_TUNE_AOS_TILES_PER_WARP, 4);
+    // row-bulk / plain: a few consecutive tiles per warp (input prefetch across tiles, staging rows reused), many CTAs per
+    // SM over the run so that the hardware CTA scheduler evens out SM-to-SM speed differences.  tile-bulk: one tile per
+    // warp measured fastest (240 vs 246 / 257 us for 1 / 2 / 4 tiles on the 128^3 grid at lmax = 9)
+    int tpw = tuned(SH_TUNE_AOS_TILES_PER_WARP, MODE == MODE_TILEBULK ? 1 : 4);
     while (tpw > 1 && ntiles / ((int64_t)WARPS * tpw) < (int64_t)sm_count() * ctas_per_sm * 4) tpw >>= 1;
     const int64_t blocks = (ntiles + (int64_t)WARPS * tpw - 1) / ((int64_t)WARPS * tpw);
     if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
-    kern<<<(unsigned)blocks, WARPS * 32, smem, st>>>(xyz, n, out, tpw, coords);
+    kern<<<(unsigned)blocks, WARPS * 32, smem, st>>>(xyz, n, out, tpw, coords, prefetch_plan(n, (int64_t)tpw * WARPS * 32));
     g_launches.fetch_add(1, std::memory_order_relaxed);
     cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? SH_OK : cuda_fail(e);
@@ -624,7 +713,7 @@ int launch_soa_pair(const float* xyz, int64_t n, float* out, int coords, cudaStr
     while (tpc > 1 && tiles / tpc < (int64_t)sm_count() * 16) tpc >>= 1;
     const int64_t blocks = (tiles + tpc - 1) / tpc;
     if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
-    sh_soa_pair_kernel<LMAX><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, out, tpc, coords);
+    sh_soa_pair_kernel<LMAX><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, out, tpc, coords, prefetch_plan(n, (int64_t)tpc * 512));
     g_launches.fetch_add(1, std::memory_order_relaxed);
     cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? SH_OK : cuda_fail(e);
@@ -661,11 +750,13 @@ int dispatch_lmax(const TI* xyz, int64_t n, T* out, int layout, int path, int co
         }
         return launch_soa<KIND, LMAX, T, TI, 8>(xyz, n, out, coords, st);
     }
-    const bool bulk_ok = aligned(out, 16) && (SP * sizeof(T)) % 16 == 0;
-    if (path == SH_STORE_BULK && !bulk_ok) return SH_ERR_ALIGNMENT;
-    if constexpr ((SP * sizeof(T)) % 16 == 0) {
-        if (bulk_ok && path != SH_STORE_DIRECT) return launch_aos<KIND, LMAX, T, TI, MODE_ROWBULK>(xyz, n, out, coords, st);
+    // bulk (TMA) paths need a 16-byte aligned `out`: one copy per warp tile where dense staging is cheap (every row size),
+    // else one copy per row (rows that are multiples of 16 B)
+    if (aligned(out, 16) && path != SH_STORE_DIRECT) {
+        if constexpr (tile_bulk_ok<KIND, LMAX, T>()) return launch_aos<KIND, LMAX, T, TI, MODE_TILEBULK>(xyz, n, out, coords, st);
+        else if constexpr ((SP * sizeof(T)) % 16 == 0) return launch_aos<KIND, LMAX, T, TI, MODE_ROWBULK>(xyz, n, out, coords, st);
     }
+    if (path == SH_STORE_BULK) return SH_ERR_ALIGNMENT;
     return launch_aos<KIND, LMAX, T, TI, MODE_PLAIN>(xyz, n, out, coords, st);
 }
 
