@@ -662,23 +662,32 @@ constexpr int aos_cap() {
     return KIND == KIND_SPINOR ? (200 > 8 * (2 * LMAX + 1) ? 200 : 8 * (2 * LMAX + 1)) : scalars_per_point(KIND, LMAX);
 }
 
-// tile-bulk mode: whole rows of a 32-point tile staged densely must fit (4 warps, 2 CTAs per SM), and the staging stores
-// must not conflict more than 2-way: 16-byte stores of a quarter warp land gcd(row_bytes/16, 8) deep; rows that are not
-// multiples of 16 B are staged with scalar stores, conflict-free because the row is then an odd number of words
+// tile-bulk mode: ONE warp per CTA (fence.proxy.async is CTA-scoped: with several warps per CTA each warp's fence also
+// waits for the other warps' copies in flight -- 4.3 vs 7.4 TB/s on a store-only model with 51.2 KB tiles), at least
+// four CTAs per SM, i.e. whole rows of a 32-point tile staged densely in <= 55 KB (complex lmax = 9: 51.2 KB), and
+// staging stores that conflict at most 4-way: 16-byte stores of a quarter warp land gcd(row_bytes/16, 8) deep; rows that
+// are not multiples of 16 B are staged with scalar stores, conflict-free because the row is then an odd number of words
+#ifndef SHB200_TILEBULK_WARPS
+#define SHB200_TILEBULK_WARPS 1
+#endif
+#ifndef SHB200_TILEBULK_MAX_CONFLICT
+#define SHB200_TILEBULK_MAX_CONFLICT 4
+#endif
+constexpr int TILEBULK_WARPS = SHB200_TILEBULK_WARPS;
 template <int KIND, int LMAX, typename T>
 constexpr bool tile_bulk_ok() {
     constexpr int row_bytes = scalars_per_point(KIND, LMAX) * (int)sizeof(T);
-    if (KIND == KIND_SPINOR || 4 * 32 * row_bytes > 110 * 1024) return false;
+    if (KIND == KIND_SPINOR || TILEBULK_WARPS * 32 * row_bytes > 55 * 1024) return false;
     if (row_bytes % 16 != 0) return true;
     int chunks = row_bytes / 16, g = 8;
     while (chunks % g) g >>= 1;
-    return g <= 2;
+    return g <= SHB200_TILEBULK_MAX_CONFLICT;
 }
 
 template <int KIND, int LMAX, typename T, typename TI, int MODE, bool ANGULAR = false>
 int launch_aos(const TI* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
     constexpr int CAP = aos_cap<KIND, LMAX>();
-    constexpr int WARPS = 4;
+    constexpr int WARPS = MODE == MODE_TILEBULK ? TILEBULK_WARPS : 4;
     using Sink = RowSink<KIND, LMAX, T, CAP, MODE>;
     constexpr size_t smem = (size_t)WARPS * 32 * Sink::PITCH * sizeof(T);
     static_assert(smem <= 227 * 1024, "staging tile exceeds shared memory");
@@ -693,10 +702,10 @@ int launch_aos(const TI* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
         ctas_per_sm = occ > 0 ? occ : 1;
     }
     const int64_t ntiles = (n + 31) / 32;
-    // row-bulk / plain: a few consecutive tiles per warp (input prefetch across tiles, staging rows reused), many CTAs per
-    // SM over the run so that the hardware CTA scheduler evens out SM-to-SM speed differences.  tile-bulk: one tile per
-    // warp measured fastest (240 vs 246 / 257 us for 1 / 2 / 4 tiles on the 128^3 grid at lmax = 9)
-    int tpw = tuned(SH_TUNE_AOS_TILES_PER_WARP, MODE == MODE_TILEBULK ? 1 : 4);
+    // one tile per warp measured fastest on every bulk path now that the input arrives by the burst L2 prefetch
+    // (real tile-bulk 238 / 242 / 249 us, spinor row-bulk 1002 / 1028 / 1064 us for 1 / 2 / 4 tiles per warp); with more
+    // tiles per warp the next tile's input is loaded before the current tile is evaluated
+    int tpw = tuned(SH_TUNE_AOS_TILES_PER_WARP, 1);
     while (tpw > 1 && ntiles / ((int64_t)WARPS * tpw) < (int64_t)sm_count() * ctas_per_sm * 4) tpw >>= 1;
     const int64_t blocks = (ntiles + (int64_t)WARPS * tpw - 1) / ((int64_t)WARPS * tpw);
     if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
@@ -709,7 +718,7 @@ int launch_aos(const TI* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
 template <int LMAX>
 int launch_soa_pair(const float* xyz, int64_t n, float* out, int coords, cudaStream_t st) {
     const int64_t tiles = ((n >> 1) + 255) / 256;
-    int tpc = tuned(SH_TUNE_SOA_TILES_PER_CTA, 2);
+    int tpc = tuned(SH_TUNE_SOA_TILES_PER_CTA, 1);
     while (tpc > 1 && tiles / tpc < (int64_t)sm_count() * 16) tpc >>= 1;
     const int64_t blocks = (tiles + tpc - 1) / tpc;
     if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
