@@ -52,7 +52,10 @@
 
 typedef long double ld;
 
-#define LMAX_CAP 9
+/* The paper's explicit formulas stop at l = 9; Eq. 5 itself and the recurrence below hold for
+ * every l, and the paper's conclusion proposes going beyond 9 by recurrence.  The cap is 32 so that
+ * this oracle can also check that extension (sh_real_ext / sh_complex_ext); nothing in the arithmetic depends on it. */
+#define LMAX_CAP 32
 #define KMAX ((LMAX_CAP + 1) * (LMAX_CAP + 1))
 
 static const ld PI_L = 3.14159265358979323846264338327950288419716939937510L;

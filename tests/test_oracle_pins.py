@@ -370,7 +370,7 @@ def test_imaginary_residue_of_eq6_vanishes(oracle_mod):
 
 def test_bad_arguments(oracle_mod):
     with pytest.raises(ValueError):
-        oracle_mod.real(np.zeros((1, 3)), 10)
+        oracle_mod.real(np.zeros((1, 3)), 33)  # the oracle's cap (32) covers the l > 9 extension
     with pytest.raises(ValueError):
         oracle_mod.real(np.zeros((1, 3)), -1)
     assert oracle_mod.real(np.zeros((0, 3)), 3).shape == (0, 16)
