@@ -204,13 +204,17 @@ def extra_configs(sh, dev):
         ("config4 complex l9 N=2^24", "complex", inputs.config4_sphere_directions(), 9, ["soa", "aos"], 3),
         ("config5 spinor l9 N=2^22", "spinor", inputs.config5_ball(), 9, ["soa", "aos"], 3),
         ("config5 real_f32 l9 N=2^22", "real_f32", inputs.config5_ball().astype(np.float32), 9, ["soa", "aos"], 20),
+        # l > 9 by recurrence: ball points of config 5, first 2^20
+        ("ext real l16 N=2^20", "real_ext", inputs.config5_ball(n=1 << 20), 16, ["soa"], 10),
+        ("ext real l32 N=2^20", "real_ext", inputs.config5_ball(n=1 << 20), 32, ["soa"], 5),
+        ("ext complex l32 N=2^20", "complex_ext", inputs.config5_ball(n=1 << 20), 32, ["soa"], 3),
     ]
     for name, kind, pts, lmax, layouts, reps in cases:
         x = torch.from_numpy(pts).to(dev)
         n = len(pts)
         per_point = sh.count(kind, lmax)
         esize = 4 if kind == "real_f32" else 8
-        values = {"real": 1, "real_f32": 1, "complex": 2, "spinor": 2}[kind]  # scalars per "value" (a complex number is one value)
+        values = {"real": 1, "real_f32": 1, "real_ext": 1, "complex": 2, "complex_ext": 2, "spinor": 2}[kind]  # scalars per "value" (a complex number is one value)
         for layout in layouts:
             out = torch.empty(sh.out_shape(kind, n, lmax, layout), dtype=x.dtype, device=dev)
             fn = getattr(sh, "sh_" + kind)

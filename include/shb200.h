@@ -93,6 +93,17 @@ int sh_spinor(const double* xyz, int64_t n, int lmax, double* out, int layout, v
 /* fp32 variant of sh_real: fp32 in, fp32 out; the normalization runs in fp64, the polynomials in fp32. */
 int sh_real_f32(const float* xyz, int64_t n, int lmax, float* out, int layout, void* stream);
 
+/* Extension beyond the paper's explicit range (its conclusion: "could be easily extended using recurrence
+ * relationships for higher values of l"): real / complex harmonics for all l <= lmax <= 32 (sh_lmax_ext()).
+ * lmax <= 9 behaves exactly like sh_real / sh_complex.  For 10 <= lmax <= 32 the explicit l <= 9 formulas seed the
+ * upward recurrence in l at fixed m of the normalized associated Legendre factors (Eq. 5 with the standard three-term
+ * recurrence), and (x + i y)^m continues by complex multiplication; same index convention k = l(l+1)+m, same r = 0
+ * convention.  SH_LAYOUT_SOA only for lmax > 9 (SH_ERR_LAYOUT otherwise); all three front ends; DEVICE pointers. */
+int sh_real_ext(const double* xyz, int64_t n, int lmax, double* out, int layout, void* stream);
+int sh_complex_ext(const double* xyz, int64_t n, int lmax, double* out, int layout, void* stream);
+/* Largest lmax the *_ext calls accept (32). */
+int sh_lmax_ext(void);
+
 /* Host-buffer entry points: same results, `xyz` and `out` are HOST pointers (pinned memory gives full
  * PCIe speed; pageable memory works).  The call copies chunks host->device, runs the kernels and copies
  * device->host on two internal streams with double buffering, and returns after `out` is complete.  The
@@ -105,12 +116,13 @@ int sh_real_f32_host(const float* xyz, int64_t n, int lmax, float* out, int layo
 /* Frees the staging buffers and streams of the host entry points (no-op if there are none). */
 void sh_host_release(void);
 
-/* Scalars (doubles for the fp64 calls, floats for sh_real_f32) written per point; -1 if lmax is out of range. */
+/* Scalars (doubles for the fp64 calls, floats for sh_real_f32) written per point; -1 if lmax is out of range
+ * (real, complex: [0, 32], the range of the *_ext calls; spinor: [0, 9]). */
 int64_t sh_real_count(int lmax);    /* K   */
 int64_t sh_complex_count(int lmax); /* 2K  */
 int64_t sh_spinor_count(int lmax);  /* 8K  */
 
-/* Element index of (l, m) in the real / complex outputs: l(l+1)+m; -1 if out of range. */
+/* Element index of (l, m) in the real / complex outputs: l(l+1)+m; -1 if out of range (l <= 32). */
 int sh_index_real(int l, int m);
 /* Element index of (l, j, m_j) in the spinor output; half-integers are passed doubled (twoj = 2j, twomj = 2m_j);
  * -1 if the triple is not a valid spin-1/2 state with l <= 9. */

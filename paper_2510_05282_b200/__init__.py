@@ -14,8 +14,11 @@ from .binding import (  # noqa: F401
     kernel_launch_count,
     load,
     out_shape,
+    lmax_ext,
     sh_complex,
+    sh_complex_ext,
     sh_real,
+    sh_real_ext,
     sh_real_f32,
     sh_spinor,
 )

@@ -48,6 +48,11 @@ def load() -> ctypes.CDLL:
             )
         lib = ctypes.CDLL(LIB_PATH)
         vp, i64, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
+        for name in ("sh_real_ext", "sh_complex_ext"):
+            f = getattr(lib, name)
+            f.argtypes = [vp, i64, ci, vp, ci, vp]
+            f.restype = ci
+        lib.sh_lmax_ext.restype = ci
         for name in ("sh_real", "sh_complex", "sh_spinor", "sh_real_f32"):
             f = getattr(lib, name)
             f.argtypes = [vp, i64, ci, vp, ci, vp]
@@ -77,7 +82,15 @@ def layout_bits(layout, store="auto", coords="cartesian") -> int:
 
 def count(kind: str, lmax: int) -> int:
     """Scalars written per point."""
-    return int(getattr(load(), f"sh_{'real' if kind == 'real_f32' else kind}_count")(lmax))
+    return int(getattr(load(), f"sh_{_BASE_KIND.get(kind, kind)}_count")(lmax))
+
+
+_BASE_KIND = {"real_f32": "real", "real_ext": "real", "complex_ext": "complex"}
+
+
+def lmax_ext() -> int:
+    """Largest lmax sh_real_ext / sh_complex_ext accept."""
+    return int(load().sh_lmax_ext())
 
 
 def index_real(l: int, m: int) -> int:
@@ -95,7 +108,7 @@ def kernel_launch_count() -> int:
 def out_shape(kind: str, n: int, lmax: int, layout) -> tuple:
     """Shape of `out` in scalars: AoS [n][K*es], SoA [K][n*es] flattened per element as [K][n][es]."""
     k = (lmax + 1) ** 2
-    es = {"real": 1, "real_f32": 1, "complex": 2, "spinor": 4}[kind]
+    es = {"real": 1, "real_f32": 1, "real_ext": 1, "complex": 2, "complex_ext": 2, "spinor": 4}[kind]
     ne = 2 * k if kind == "spinor" else k
     if _LAYOUTS[layout] == SH_LAYOUT_AOS:
         return (n, ne, es) if es > 1 else (n, ne)
@@ -143,6 +156,16 @@ def sh_spinor(xyz, lmax, out=None, layout="soa", store="auto", stream=None, coor
 def sh_real_f32(xyz, lmax, out=None, layout="soa", store="auto", stream=None, coords="cartesian"):
     """fp32 variant of sh_real (float32 in, float32 out)."""
     return _device_call("real_f32", xyz, lmax, out, layout, store, stream, coords)
+
+
+def sh_real_ext(xyz, lmax, out=None, layout="soa", store="auto", stream=None, coords="cartesian"):
+    """R_l^m for l <= lmax <= 32: the explicit l <= 9 block plus the recurrence extension.  SoA only for lmax > 9."""
+    return _device_call("real_ext", xyz, lmax, out, layout, store, stream, coords)
+
+
+def sh_complex_ext(xyz, lmax, out=None, layout="soa", store="auto", stream=None, coords="cartesian"):
+    """Y_l^m for l <= lmax <= 32 (see sh_real_ext)."""
+    return _device_call("complex_ext", xyz, lmax, out, layout, store, stream, coords)
 
 
 def host_call(kind: str, xyz: "np.ndarray | object", lmax: int, out=None, layout="soa", coords="cartesian"):

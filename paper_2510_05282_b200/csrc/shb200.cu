@@ -25,6 +25,7 @@
 
 #include "../../include/shb200.h"
 #define SHGEN_FN __device__ __forceinline__
+#define SHGEN_TABLE __constant__   /* recurrence tables of the l > 9 extension live in constant memory */
 #include "sh_generated.cuh"
 
 namespace {
@@ -183,8 +184,7 @@ struct Azim {
 };
 
 template <int LMAX, typename T, class O, class Sink>
-__device__ __forceinline__ void eval_real(T x, T y, T z, O origin, Sink& sink) {
-    const Azim<LMAX, T> az(x, y);
+__device__ __forceinline__ void eval_real(const Azim<LMAX, T>& az, T z, O origin, Sink& sink) {
     static_for<0, LMAX + 1>([&](auto lc) {
         constexpr int L = decltype(lc)::value;
         T q[L + 1];
@@ -195,6 +195,7 @@ __device__ __forceinline__ void eval_real(T x, T y, T z, O origin, Sink& sink) {
         });
         // r = 0: x = y = z = 0 zeroes everything except the even-l, m = 0 polynomials (P_l(0) != 0)
         if constexpr (L > 0 && L % 2 == 0) q[0] = zero_where(origin, q[0]);
+        sink.template polar<L>(q);   // the normalized polar factors of block l (seeds of the l > 9 recurrence)
         static_for<0, L>([&](auto jc) {
             constexpr int M = L - decltype(jc)::value;
             sink.template put1<L * (L + 1) - M>(q[M] * az.S[M]);
@@ -208,26 +209,36 @@ __device__ __forceinline__ void eval_real(T x, T y, T z, O origin, Sink& sink) {
     });
 }
 
+template <int LMAX, typename T, class O, class Sink>
+__device__ __forceinline__ void eval_real(T x, T y, T z, O origin, Sink& sink) {
+    const Azim<LMAX, T> az(x, y);
+    eval_real<LMAX, T>(az, z, origin, sink);
+}
+
 // a[M] + i b[M] = B_lm Qhat_lm (C_M + i S_M);  Y_l^{-M} = (a, -b),  Y_l^{+M} = (-1)^M (a, b)
-template <int L, int LMAX, typename T>
-__device__ __forceinline__ void complex_block(const Azim<LMAX, T>& az, T z, bool origin, T (&a)[L + 1], T (&b)[L + 1]) {
+template <int L, int LMAX, typename T, class Sink>
+__device__ __forceinline__ void complex_block(const Azim<LMAX, T>& az, T z, bool origin, T (&a)[L + 1], T (&b)[L + 1], Sink& sink) {
+    T u[L + 1];
     static_for<0, L + 1>([&](auto mc) {
         constexpr int M = decltype(mc)::value;
         constexpr double B = shgen::B_CPLX[L][M];
-        const T u = T(B) * shgen::Polar<L, M, T>::eval(z);
-        a[M] = u * az.C[M];
-        b[M] = u * az.S[M];
+        u[M] = T(B) * shgen::Polar<L, M, T>::eval(z);
     });
-    if constexpr (L > 0 && L % 2 == 0) a[0] = zero_where(origin, a[0]);
+    if constexpr (L > 0 && L % 2 == 0) u[0] = zero_where(origin, u[0]);
+    sink.template polar<L>(u);
+    static_for<0, L + 1>([&](auto mc) {
+        constexpr int M = decltype(mc)::value;
+        a[M] = u[M] * az.C[M];
+        b[M] = u[M] * az.S[M];
+    });
 }
 
 template <int LMAX, typename T, class Sink>
-__device__ __forceinline__ void eval_complex(T x, T y, T z, bool origin, Sink& sink) {
-    const Azim<LMAX, T> az(x, y);
+__device__ __forceinline__ void eval_complex(const Azim<LMAX, T>& az, T z, bool origin, Sink& sink) {
     static_for<0, LMAX + 1>([&](auto lc) {
         constexpr int L = decltype(lc)::value;
         T a[L + 1], b[L + 1];
-        complex_block<L>(az, z, origin, a, b);
+        complex_block<L>(az, z, origin, a, b, sink);
         static_for<0, L>([&](auto jc) {
             constexpr int M = L - decltype(jc)::value;
             sink.template put2<L * (L + 1) - M>(a[M], -b[M]);
@@ -240,6 +251,12 @@ __device__ __forceinline__ void eval_complex(T x, T y, T z, bool origin, Sink& s
         });
         sink.template end_l<L>();
     });
+}
+
+template <int LMAX, typename T, class Sink>
+__device__ __forceinline__ void eval_complex(T x, T y, T z, bool origin, Sink& sink) {
+    const Azim<LMAX, T> az(x, y);
+    eval_complex<LMAX, T>(az, z, origin, sink);
 }
 
 // component c * Y_l^m from the block's (a, b); c and the signs fold into one compile-time constant
@@ -264,7 +281,7 @@ __device__ __forceinline__ void eval_spinor(T x, T y, T z, bool origin, Sink& si
     static_for<0, LMAX + 1>([&](auto lc) {
         constexpr int L = decltype(lc)::value;
         T a[L + 1], b[L + 1];
-        complex_block<L>(az, z, origin, a, b);
+        complex_block<L>(az, z, origin, a, b, sink);
         static_for<2 * L * L, 2 * (L + 1) * (L + 1)>([&](auto sc) {
             constexpr int S = decltype(sc)::value;
             constexpr shgen::SpinorEntry e = shgen::SPINOR[S];
@@ -318,6 +335,7 @@ struct SoASink {
         } else { __stcs(q, a); __stcs(q + 1, b); __stcs(q + 2, c); __stcs(q + 3, d); }
     }
     template <int L> __device__ __forceinline__ void end_l() {}
+    template <int L> __device__ __forceinline__ void polar(const T (&)[L + 1]) {}
 };
 
 template <int KIND, int LMAX, typename T, typename TI, int VEC, bool ANGULAR>
@@ -351,6 +369,7 @@ struct SoAPairSink {
     int64_t stride;   // n
     template <int K> __device__ __forceinline__ void put1(f2 v) { __stcs(reinterpret_cast<float2*>(p + K * stride), v.v); }
     template <int L> __device__ __forceinline__ void end_l() {}
+    template <int L> __device__ __forceinline__ void polar(const f2 (&)[L + 1]) {}
 };
 
 template <int LMAX>
@@ -378,6 +397,98 @@ __global__ void __launch_bounds__(256) sh_soa_pair_kernel(const float* __restric
         }
         ca = na; cb = nb; cc = nc;
         have = have_next;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Extension beyond the explicit range, 10 <= l <= LMAX_EXT = 32 (the paper's conclusion: "could be easily
+// extended using recurrence relationships for higher values of l").  The explicit l <= 9 block is evaluated as above
+// and seeds, at fixed m, the upward recurrence in l of the normalized polar factors (tables from the generator):
+//   q_lm = A_lm (z q_{l-1,m} - B_lm q_{l-2,m})   seeds q_8m, q_9m (m <= 9);      q_ll = SECT_l q_{l-1,l-1}  (l >= 10)
+//   C_m + i S_m = (C_{m-1} + i S_{m-1}) (x + i y)                                 seeds C_9, S_9            (m >= 10)
+// Loops run m-outer, l-inner, so a thread carries two q's and one (C_m, S_m) only; SoA planes make every store of a
+// warp contiguous whatever the order of (l, m).  (AoS rows would be written 8 bytes at a time, columns l(l+1)+-m
+// far apart: not offered for lmax > 9.)
+template <int KIND>
+struct SoAExtSink {
+    double* p;        // out + i*ES
+    int64_t stride;   // n*ES
+    bool vec16;       // complex elements may be written by one 16-byte store
+    double q8[9], q9[10];
+    template <int K> __device__ __forceinline__ void put1(double v) { __stcs(p + K * stride, v); }
+    template <int K> __device__ __forceinline__ void put2(double re, double im) { put_complex(K, re, im); }
+    template <int L> __device__ __forceinline__ void end_l() {}
+    template <int L> __device__ __forceinline__ void polar(const double (&q)[L + 1]) {
+        if constexpr (L == 8) { static_for<0, 9>([&](auto mc) { q8[decltype(mc)::value] = q[decltype(mc)::value]; }); }
+        if constexpr (L == 9) { static_for<0, 10>([&](auto mc) { q9[decltype(mc)::value] = q[decltype(mc)::value]; }); }
+    }
+    __device__ __forceinline__ void put_complex(int k, double re, double im) {
+        double* q = p + k * stride;
+        if (vec16) __stcs(reinterpret_cast<double2*>(q), make_double2(re, im));
+        else { __stcs(q, re); __stcs(q + 1, im); }
+    }
+    // harmonics (l, +-m) from the polar factor q and the azimuthal pair (c, s); KIND_REAL: Eq. 6; KIND_COMPLEX: Eq. 5, 10
+    __device__ __forceinline__ void emit(int l, int m, double q, double c, double s) {
+        const int k0 = l * (l + 1);
+        if constexpr (KIND == KIND_REAL) {
+            if (m == 0) { __stcs(p + k0 * stride, q); return; }
+            __stcs(p + (k0 + m) * stride, q * c);
+            __stcs(p + (k0 - m) * stride, q * s);
+        } else {
+            if (m == 0) { put_complex(k0, q, 0.0); return; }
+            const double a = q * c, b = q * s;
+            put_complex(k0 - m, a, -b);
+            if (m & 1) put_complex(k0 + m, -a, -b);
+            else put_complex(k0 + m, a, b);
+        }
+    }
+};
+
+template <int KIND, bool ANGULAR>
+__global__ void __launch_bounds__(256) sh_soa_ext_kernel(const double* __restrict__ xyz, int64_t n, double* __restrict__ out, int lmax, int coords, int vec16,
+                                                          InputPrefetch pf) {
+    constexpr int ES = elem_scalars(KIND);
+    constexpr int IN_BYTES = (ANGULAR ? 2 : 3) * sizeof(double);
+    constexpr int NT = shgen::LMAX_EXT + 1;
+    prefetch_input_window(xyz, n * IN_BYTES, (int64_t)256 * IN_BYTES, pf);
+    const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (i >= n) return;
+    RawPoint<double, ANGULAR> pt;
+    pt.load(xyz, i);
+    const UnitVec u = pt.unit(coords);
+    const double z = u.z;
+    SoAExtSink<KIND> sink;
+    sink.p = out + i * ES;
+    sink.stride = n * ES;
+    sink.vec16 = vec16 != 0;
+    const Azim<9, double> az(u.x, u.y);
+    if constexpr (KIND == KIND_REAL) eval_real<9, double>(az, z, u.origin, sink);
+    else eval_complex<9, double>(az, z, u.origin, sink);
+    // m <= 9: the explicit factors C_m, S_m; l = 10 .. lmax by recurrence from the explicit q_8m, q_9m
+    static_for<0, 10>([&](auto mc) {
+        constexpr int M = decltype(mc)::value;
+        double q2 = 0.0, q1 = sink.q9[M];
+        if constexpr (M <= 8) q2 = sink.q8[M];
+        for (int l = 10; l <= lmax; ++l) {
+            const double q = shgen::REC_A[l * NT + M] * (z * q1 - shgen::REC_B[l * NT + M] * q2);
+            sink.emit(l, M, q, az.C[M], az.S[M]);
+            q2 = q1; q1 = q;
+        }
+    });
+    // m >= 10: sectoral seed q_mm, azimuthal pair by complex multiplication, then the same recurrence in l
+    double c = az.C[9], s = az.S[9], qmm = sink.q9[9];
+    for (int m = 10; m <= lmax; ++m) {
+        const double cn = c * u.x - s * u.y;
+        s = c * u.y + s * u.x;
+        c = cn;
+        qmm *= shgen::REC_SECT[m];
+        sink.emit(m, m, qmm, c, s);
+        double q2 = 0.0, q1 = qmm;
+        for (int l = m + 1; l <= lmax; ++l) {
+            const double q = shgen::REC_A[l * NT + m] * (z * q1 - shgen::REC_B[l * NT + m] * q2);
+            sink.emit(l, m, q, c, s);
+            q2 = q1; q1 = q;
+        }
     }
 }
 
@@ -486,6 +597,8 @@ struct RowSink {
         if constexpr (!VSTAGE) { row[O] = a; row[O + 1] = b; row[O + 2] = c; row[O + 3] = d; }
         else { st16(row + O, a, b); st16(row + O + 2, c, d); }
     }
+
+    template <int L> __device__ __forceinline__ void polar(const T (&)[L + 1]) {}
 
     __device__ __forceinline__ void wait_reads() {
         if constexpr (MODE != MODE_PLAIN) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
@@ -792,6 +905,30 @@ int run_device(const TI* xyz, int64_t n, int lmax, T* out, int layout_bits, void
     return SH_ERR_LMAX;
 }
 
+// l > 9 extension (sh_real_ext / sh_complex_ext): lmax <= 9 is the regular path; above, SoA only
+template <int KIND>
+int run_device_ext(const double* xyz, int64_t n, int lmax, double* out, int layout_bits, void* stream) {
+    if (lmax <= shgen::LMAX_CAP) return run_device<KIND, double, double>(xyz, n, lmax, out, layout_bits, stream);
+    if (n < 0) return SH_ERR_COUNT;
+    if (lmax > shgen::LMAX_EXT) return SH_ERR_LMAX;
+    const int layout = layout_bits & 0xff, path = layout_bits & 0xff00, coords = layout_bits & 0x30000;
+    if ((layout_bits & ~0x3ffff) || layout != SH_LAYOUT_SOA || (path != SH_STORE_AUTO && path != SH_STORE_DIRECT) || coords == 0x30000)
+        return SH_ERR_LAYOUT;
+    if (n == 0) return SH_OK;
+    if (!xyz || !out) return SH_ERR_NULL;
+    if (!aligned(out, sizeof(double)) || !aligned(xyz, sizeof(double))) return SH_ERR_ALIGNMENT;
+    const int64_t blocks = (n + 255) / 256;
+    if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int vec16 = aligned(out, 16) ? 1 : 0;   // complex element (k*n + i) sits 16 (k*n + i) bytes into `out`
+    const InputPrefetch pf = prefetch_plan(n, 256);
+    if (coords == SH_COORDS_ANGULAR) sh_soa_ext_kernel<KIND, true><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, out, lmax, coords, vec16, pf);
+    else sh_soa_ext_kernel<KIND, false><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, out, lmax, coords, vec16, pf);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? SH_OK : cuda_fail(e);
+}
+
 // Host-buffer pipeline: chunks of points go host -> device -> kernel -> host on two streams (double buffering):
 // the device->host copy of chunk c overlaps the host->device copy and the kernel of chunk c+1.
 // The two staging slots (64 MiB input + 256 MiB output each) and their streams are created on first use and
@@ -891,6 +1028,14 @@ int sh_real_f32(const float* xyz, int64_t n, int lmax, float* out, int layout, v
     return run_device<KIND_REAL, float, float>(xyz, n, lmax, out, layout, stream);
 }
 
+int sh_real_ext(const double* xyz, int64_t n, int lmax, double* out, int layout, void* stream) {
+    return run_device_ext<KIND_REAL>(xyz, n, lmax, out, layout, stream);
+}
+int sh_complex_ext(const double* xyz, int64_t n, int lmax, double* out, int layout, void* stream) {
+    return run_device_ext<KIND_COMPLEX>(xyz, n, lmax, out, layout, stream);
+}
+int sh_lmax_ext(void) { return shgen::LMAX_EXT; }
+
 int sh_real_host(const double* xyz, int64_t n, int lmax, double* out, int layout) {
     return run_host<KIND_REAL, double, double>(xyz, n, lmax, out, layout);
 }
@@ -909,12 +1054,12 @@ void sh_host_release(void) {
     g_pool.release();
 }
 
-int64_t sh_real_count(int lmax) { return (lmax < 0 || lmax > 9) ? -1 : (int64_t)(lmax + 1) * (lmax + 1); }
-int64_t sh_complex_count(int lmax) { return (lmax < 0 || lmax > 9) ? -1 : 2 * (int64_t)(lmax + 1) * (lmax + 1); }
+int64_t sh_real_count(int lmax) { return (lmax < 0 || lmax > shgen::LMAX_EXT) ? -1 : (int64_t)(lmax + 1) * (lmax + 1); }
+int64_t sh_complex_count(int lmax) { return (lmax < 0 || lmax > shgen::LMAX_EXT) ? -1 : 2 * (int64_t)(lmax + 1) * (lmax + 1); }
 int64_t sh_spinor_count(int lmax) { return (lmax < 0 || lmax > 9) ? -1 : 8 * (int64_t)(lmax + 1) * (lmax + 1); }
 
 int sh_index_real(int l, int m) {
-    if (l < 0 || l > 9 || m < -l || m > l) return -1;
+    if (l < 0 || l > shgen::LMAX_EXT || m < -l || m > l) return -1;
     return l * (l + 1) + m;
 }
 
@@ -932,8 +1077,8 @@ const char* sh_strerror(int code) {
         case SH_OK: return "ok";
         case SH_ERR_NULL: return "xyz or out is NULL with n > 0";
         case SH_ERR_COUNT: return "n is negative or too large for one launch";
-        case SH_ERR_LMAX: return "lmax must be in [0, 9]";
-        case SH_ERR_LAYOUT: return "unknown layout or store-path bits";
+        case SH_ERR_LMAX: return "lmax must be in [0, 9] (sh_real_ext / sh_complex_ext: [0, 32])";
+        case SH_ERR_LAYOUT: return "unknown layout, store-path or front-end bits, or a layout this call does not offer";
         case SH_ERR_ALIGNMENT: return "pointer not aligned to its element type, or requested store path impossible for this alignment";
         case SH_ERR_CUDA: return "CUDA error (see sh_last_cuda_error)";
     }

@@ -29,6 +29,15 @@ aborts on any mismatch > 1e-45.
 The spinor table follows Eq. 7: for l = j -+ 1/2,
   up   = +-sqrt(l +- m_j + 1/2)/sqrt(2l+1) * Y_l^{m_j-1/2},   down = sqrt(l -+ m_j + 1/2)/sqrt(2l+1) * Y_l^{m_j+1/2}.
 
+Beyond the explicit range (the paper's conclusion: "could be easily extended using recurrence
+relationships for higher values of l"), for 10 <= l <= 32 the script emits the coefficient tables of the upward
+recurrence in l at fixed m for the normalized polar factors q_lm = f_m K_l^m Q_l^m(z) (f_0 = 1, f_m = sqrt2):
+
+  q_lm = A_lm (z q_{l-1,m} - B_lm q_{l-2,m}),   A_lm = sqrt((4l^2-1)/(l^2-m^2)),  B_lm = sqrt(((l-1)^2-m^2)/(4(l-1)^2-1))
+  q_ll = sqrt((2l+1)/(2l)) q_{l-1,l-1}                                                        (l >= 2)
+
+seeded by the explicit l = 8, 9 block, and checks them against the closed forms above before writing.
+
 This file shares no code with oracle/ (which never evaluates a polynomial in x, y, z).
 Usage: python generate.py [output.cuh]
 """
@@ -43,6 +52,7 @@ import mpmath as mp
 
 mp.mp.dps = 60
 LMAX = 9
+LMAX_EXT = 32   # reach of the recurrence extension
 
 
 # ----------------------------------------------------------------------------- closed forms
@@ -137,6 +147,38 @@ def self_check():
                 assert abs(val - ref) < mp.mpf(10) ** -25 * max(1, abs(ref)), ("polar/mpmath", l, m)
                 exact = sum((mp.mpf(c.numerator) / c.denominator) * z**k for k, c in enumerate(q_poly(l, m)))
                 assert abs(val - exact) < tol * max(1, abs(exact)), ("polar/exact", l, m)
+
+
+# ----------------------------------------------------------------------------- recurrence extension, l > 9
+def rec_a(l: int, m: int):
+    return mp.sqrt(mp.mpf(4 * l * l - 1) / mp.mpf(l * l - m * m))
+
+
+def rec_b(l: int, m: int):
+    return mp.sqrt(mp.mpf((l - 1) ** 2 - m * m) / mp.mpf(4 * (l - 1) ** 2 - 1))
+
+
+def rec_sect(l: int):
+    return mp.sqrt(mp.mpf(2 * l + 1) / mp.mpf(2 * l))
+
+
+def self_check_recurrence():
+    """q_lm = f_m K_l^m Q_l^m(z) from the exact Legendre coefficients obeys the emitted recurrences for every l <= LMAX_EXT."""
+    tol = mp.mpf(10) ** -40
+
+    def q(l, m, z):
+        if m > l:
+            return mp.mpf(0)
+        val = sum((mp.mpf(c.numerator) / c.denominator) * z**k for k, c in enumerate(q_poly(l, m)))
+        return (mp.sqrt(2) if m else 1) * K(l, m) * val
+
+    for z in (mp.mpf("0.31"), mp.mpf("-0.95")):
+        for l in range(2, LMAX_EXT + 1):
+            assert abs(q(l, l, z) - rec_sect(l) * q(l - 1, l - 1, z)) < tol * abs(q(l, l, z)), ("sectoral", l)
+            for m in range(l):
+                want = q(l, m, z)
+                got = rec_a(l, m) * (z * q(l - 1, m, z) - rec_b(l, m) * q(l - 2, m, z))
+                assert abs(got - want) < tol * max(1, abs(want)), ("recurrence", l, m)
 
 
 # ----------------------------------------------------------------------------- emission
@@ -252,6 +294,21 @@ def emit() -> str:
         w(f"    {{{l}, {twoj}, {twomj}, {m_up}, {m_dn}, {dlit(cu)}, {dlit(cd)}}},")
     w("};")
     w("")
+    w("// ---- recurrence extension, 10 <= l <= 32 (PAPER.md line 183): q_lm = REC_A (z q_{l-1,m} - REC_B q_{l-2,m}), m < l;")
+    w("// q_ll = REC_SECT[l] q_{l-1,l-1}; q_lm = f_m K_l^m Q_l^m(z), seeded by the explicit l = 8, 9 block.  Index [l * 33 + m].")
+    w(f"constexpr int LMAX_EXT = {LMAX_EXT};")
+    w("#ifndef SHGEN_TABLE")
+    w("#define SHGEN_TABLE static const")
+    w("#endif")
+    n1 = LMAX_EXT + 1
+    for name, fn in (("REC_A", rec_a), ("REC_B", rec_b)):
+        w(f"SHGEN_TABLE double {name}[{n1} * {n1}] = {{")
+        for l in range(n1):
+            row = [dlit(fn(l, m)) if (l >= 2 and m < l) else "0.0" for m in range(n1)]
+            w("    " + ", ".join(row) + ",")
+        w("};")
+    w(f"SHGEN_TABLE double REC_SECT[{n1}] = {{" + ", ".join(dlit(rec_sect(l)) if l >= 2 else "0.0" for l in range(n1)) + "};")
+    w("")
     w("}  // namespace shgen")
     w("")
     return "\n".join(o)
@@ -261,6 +318,7 @@ def main(argv):
     here = os.path.dirname(os.path.abspath(__file__))
     out = argv[1] if len(argv) > 1 else os.path.join(here, "..", "csrc", "sh_generated.cuh")
     self_check()
+    self_check_recurrence()
     text = emit()
     out = os.path.abspath(out)
     if not os.path.exists(out) or open(out).read() != text:

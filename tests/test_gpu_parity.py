@@ -405,3 +405,68 @@ def test_accuracy_study_like_fig1(sh, oracle_mod):
     os.makedirs("gpurun_out", exist_ok=True)
     with open(os.path.join("gpurun_out", "accuracy_study.txt"), "w") as f:
         f.write(report + "\n")
+
+
+# ----------------------------------------------------------------------------- l > 9 by recurrence
+@pytest.mark.parametrize("kind", ["real_ext", "complex_ext"])
+def test_ext_all_lmax_up_to_32(sh, oracle_mod, cube_points, kind):
+    """sh_real_ext / sh_complex_ext, every lmax in [0, 32], config-1 points (r = 0, poles, axes, ragged tail)."""
+    assert sh.lmax_ext() == 32
+    worst = 0.0
+    for lmax in list(range(0, 13)) + [16, 21, 27, 31, 32]:
+        for layout in (["soa", "aos"] if lmax <= 9 else ["soa"]):
+            got = gpu_eval(sh, kind, cube_points, lmax, layout)
+            want = oracle_eval(oracle_mod, kind.replace("_ext", ""), cube_points, lmax)
+            assert got.shape == want.shape
+            worst = max(worst, max_err(got, want))
+    assert worst <= TOL64, worst
+
+
+def test_ext_front_ends_near_poles_misalignment_and_refusals(sh, oracle_mod):
+    rng = np.random.default_rng(32)
+    pts = []
+    for s in (1e-2, 1e-5, 1e-9):
+        for _ in range(6):
+            phi = rng.uniform(-np.pi, np.pi)
+            pts.append([s * np.cos(phi), s * np.sin(phi), rng.choice([-1.0, 1.0])])
+    pts = np.concatenate([np.array(pts) * 2.0, rng.uniform(-3, 3, (515, 3)), rng.standard_normal((64, 3)) * 1e-200])
+    for kind in ("real_ext", "complex_ext"):
+        base = kind.replace("_ext", "")
+        for mis in (0, 1):  # 8-byte aligned out: scalar stores for complex elements
+            got = gpu_eval(sh, kind, pts, 32, "soa", misalign=mis)
+            assert max_err(got, oracle_eval(oracle_mod, base, pts, 32)) <= TOL64, (kind, mis)
+        unit = pts[:-64] / np.linalg.norm(pts[:-64], axis=1)[:, None]  # (numpy's norm underflows on the 1e-200 points)
+        got = gpu_eval(sh, kind, unit, 20, "soa", coords="normalized")
+        assert max_err(got, oracle_eval(oracle_mod, base, unit, 20)) <= TOL64
+        tp = np.stack([rng.uniform(0, np.pi, 700), rng.uniform(-np.pi, np.pi, 700)], axis=1)
+        tp[:2] = [[0.0, 1.0], [np.pi, -1.0]]
+        got = gpu_eval(sh, kind, tp, 32, "soa", coords="angular")
+        want = oracle_mod.real_angular(tp, 32) if base == "real" else oracle_mod.complex_angular(tp, 32).view(np.float64).reshape(700, -1, 2)
+        assert max_err(got, want) <= TOL64
+        with pytest.raises(sh.ShError):  # AoS is not offered above lmax = 9
+            gpu_eval(sh, kind, pts, 10, "aos")
+        with pytest.raises(sh.ShError):
+            gpu_eval(sh, kind, pts, 33, "soa")
+
+
+def test_ext_full_size_sampled_and_unsoeld(sh, oracle_mod):
+    """lmax = 32 on 2^20 points of the config-5 ball (9.1 GB of output, the bench's launch configuration): sampled points
+    against the oracle, and the addition theorem at every point and every l."""
+    import torch
+    from paper_2510_05282_b200 import inputs
+
+    pts = inputs.config5_ball(n=1 << 20)
+    n = len(pts)
+    x = torch.from_numpy(pts).cuda()
+    out = sh.sh_real_ext(x, 32, layout="soa")
+    torch.cuda.synchronize()
+    idx = sample_indices(n, 3000, 61)
+    got = out[:, torch.from_numpy(idx).cuda()].t().contiguous().cpu().numpy()
+    assert max_err(got, oracle_mod.real(pts[idx], 32)) <= TOL64
+    # every value within TOL64 of the truth => |sum_m R^2 - (2l+1)/4pi| <= 2 sqrt((2l+1)/4pi) sqrt(2l+1) TOL64 (Cauchy-Schwarz).
+    # The largest value error is inherent in fp64 coordinates: near the poles dR_l^0/dz = K_l^0 l(l+1)/2 ~ 1.2e3 at l = 32, so
+    # one ulp of z/r is already 1.3e-13 (observed: 2.8e-13 at l = 32, m = 0, |z/r| = 0.9997; 1.1e-14 at l = 9).
+    for l in range(33):
+        dens = (out[l * l : (l + 1) ** 2] ** 2).sum(dim=0)
+        bound = 2 * np.sqrt((2 * l + 1) / (4 * np.pi)) * np.sqrt(2 * l + 1) * TOL64
+        assert float((dens - (2 * l + 1) / (4 * np.pi)).abs().max()) <= bound, l

@@ -35,9 +35,12 @@ def test_counts_and_indices(lib):
     for lmax in range(10):
         k = (lmax + 1) ** 2
         assert lib.sh_real_count(lmax) == k and lib.sh_complex_count(lmax) == 2 * k and lib.sh_spinor_count(lmax) == 8 * k
-    assert lib.sh_real_count(10) == -1 and lib.sh_spinor_count(-1) == -1
-    assert [lib.sh_index_real(l, m) for l in range(10) for m in range(-l, l + 1)] == list(range(100))
-    assert lib.sh_index_real(3, 4) == -1 and lib.sh_index_real(10, 0) == -1
+    # real / complex counts and indices reach l = 32, the range of sh_real_ext / sh_complex_ext; spinors stop at 9
+    assert lib.sh_lmax_ext() == 32
+    assert lib.sh_real_count(32) == 1089 and lib.sh_complex_count(32) == 2178
+    assert lib.sh_real_count(33) == -1 and lib.sh_spinor_count(10) == -1 and lib.sh_spinor_count(-1) == -1
+    assert [lib.sh_index_real(l, m) for l in range(33) for m in range(-l, l + 1)] == list(range(1089))
+    assert lib.sh_index_real(3, 4) == -1 and lib.sh_index_real(33, 0) == -1
     seen = []
     for l in range(10):
         for twoj in (2 * l - 1, 2 * l + 1):
@@ -64,6 +67,12 @@ def test_argument_validation_without_gpu(lib):
         assert fn(p, 4, 3, None, 1, None) == -1
         assert fn(None, 0, 3, None, 0, None) == 0        # n = 0: successful no-op
     assert lib.sh_real(p, 4, 3, p + 4, 0, None) == -5    # SH_ERR_ALIGNMENT
+    for fn in (lib.sh_real_ext, lib.sh_complex_ext):
+        assert fn(p, -1, 20, p, 1, None) == -2 and fn(p, 4, 33, p, 1, None) == -3 and fn(p, 4, -1, p, 1, None) == -3
+        assert fn(p, 4, 10, p, 0, None) == -4            # AoS is not offered above lmax = 9
+        assert fn(p, 4, 20, p, 1 | (2 << 8), None) == -4  # nor the bulk store path
+        assert fn(None, 4, 20, p, 1, None) == -1 and fn(None, 0, 20, None, 1, None) == 0
+        assert fn(p, 4, 20, p + 4, 1, None) == -5
     for fn in (lib.sh_real_host, lib.sh_complex_host, lib.sh_spinor_host, lib.sh_real_f32_host):
         assert fn(p, -1, 3, p, 0) == -2 and fn(p, 1, 11, p, 0) == -3 and fn(None, 0, 3, None, 1) == 0
     for code in range(-6, 1):
@@ -85,5 +94,6 @@ def test_generator_output_is_current():
     from paper_2510_05282_b200.gen import generate
 
     generate.self_check()
+    generate.self_check_recurrence()
     path = os.path.join(ROOT, "paper_2510_05282_b200", "csrc", "sh_generated.cuh")
     assert open(path).read() == generate.emit()
