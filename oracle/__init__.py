@@ -45,6 +45,13 @@ def _load():
         lib.sh_oracle_max_imag_residue.restype = ctypes.c_double
         lib.sh_oracle_index_spinor.argtypes = [ctypes.c_int] * 3
         lib.sh_oracle_index_spinor.restype = ctypes.c_int
+        ip = ctypes.POINTER(ctypes.c_int)
+        lib.sh_oracle_projector_count.argtypes = [ctypes.c_int, ip]
+        lib.sh_oracle_projector_count.restype = ctypes.c_int
+        lib.sh_oracle_projectors.argtypes = [dp, ctypes.c_int64, ctypes.c_int, ip, dp, ctypes.c_int, ctypes.c_double, dp]
+        lib.sh_oracle_projectors.restype = ctypes.c_int
+        lib.sh_oracle_project.argtypes = [dp, ctypes.c_int64, ctypes.c_int, ip, dp, ctypes.c_int, ctypes.c_double, dp, ctypes.c_int, dp, dp]
+        lib.sh_oracle_project.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -123,3 +130,53 @@ def max_imag_residue() -> float:
 
 def reset_imag_residue() -> None:
     _load().sh_oracle_reset_imag_residue()
+
+
+# ---- fused projector consumer (definition in sh_oracle.c) ----
+def _proj_args(xyz, proj_l, radial, dr):
+    a = np.ascontiguousarray(xyz, dtype=np.float64)
+    if a.ndim != 2 or a.shape[1] != 3:
+        raise ValueError("expected [n][3] array")
+    pl = np.ascontiguousarray(proj_l, dtype=np.int32)
+    tab = np.ascontiguousarray(radial, dtype=np.float64)
+    if tab.ndim != 2 or tab.shape[0] != len(pl):
+        raise ValueError("radial must be [nproj][nr]")
+    return a, pl, tab, float(dr)
+
+
+def projector_count(proj_l) -> int:
+    """ncols = sum_p (2 l_p + 1)."""
+    pl = np.ascontiguousarray(proj_l, dtype=np.int32)
+    return _load().sh_oracle_projector_count(len(pl), pl.ctypes.data_as(ctypes.POINTER(ctypes.c_int)))
+
+
+def projectors(xyz, proj_l, radial, dr):
+    """beta_{p,m}(r_i) = f_p(|r_i|) R_{l_p}^m(r_i/|r_i|): [n][ncols] float64 (columns channel-major, m ascending)."""
+    a, pl, tab, dr = _proj_args(xyz, proj_l, radial, dr)
+    ncols = projector_count(pl)
+    out = np.empty((len(a), ncols), dtype=np.float64)
+    dp, ip = ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int)
+    rc = _load().sh_oracle_projectors(a.ctypes.data_as(dp), len(a), len(pl), pl.ctypes.data_as(ip), tab.ctypes.data_as(dp),
+                                      tab.shape[1], dr, out.ctypes.data_as(dp))
+    if rc != 0:
+        raise ValueError("sh_oracle_projectors: bad arguments")
+    return out
+
+
+def project(xyz, proj_l, radial, dr, w):
+    """coeff[v][col] = sum_i w[v][i] beta_col(r_i) (plain long-double sum in point order) and the sums of |terms|:
+    returns (coeff, abs_sum), both [nvec][ncols] float64."""
+    a, pl, tab, dr = _proj_args(xyz, proj_l, radial, dr)
+    ww = np.ascontiguousarray(w, dtype=np.float64)
+    if ww.ndim != 2 or ww.shape[1] != len(a):
+        raise ValueError("w must be [nvec][n]")
+    ncols = projector_count(pl)
+    coeff = np.empty((ww.shape[0], ncols), dtype=np.float64)
+    abs_sum = np.empty_like(coeff)
+    dp, ip = ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int)
+    rc = _load().sh_oracle_project(a.ctypes.data_as(dp), len(a), len(pl), pl.ctypes.data_as(ip), tab.ctypes.data_as(dp),
+                                   tab.shape[1], dr, ww.ctypes.data_as(dp), ww.shape[0], coeff.ctypes.data_as(dp),
+                                   abs_sum.ctypes.data_as(dp))
+    if rc != 0:
+        raise ValueError("sh_oracle_project: bad arguments")
+    return coeff, abs_sum

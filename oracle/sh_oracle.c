@@ -46,6 +46,7 @@
 #include <math.h>
 #include <stdint.h>
 #include <stddef.h>
+#include <stdlib.h>
 #ifdef _OPENMP
 #include <omp.h>
 #endif
@@ -258,3 +259,101 @@ int sh_oracle_spinor(const double* xyz, int64_t n, int lmax, double* out) { retu
 int sh_oracle_real_angular(const double* tp, int64_t n, int lmax, double* out) { return run(0, 1, tp, n, lmax, out); }
 int sh_oracle_complex_angular(const double* tp, int64_t n, int lmax, double* out) { return run(1, 1, tp, n, lmax, out); }
 int sh_oracle_spinor_angular(const double* tp, int64_t n, int lmax, double* out) { return run(2, 1, tp, n, lmax, out); }
+
+/* ------------------------------------------------------------------------------------------------
+ * Fused projector consumer (the use case of PAPER.md lines 14 and 20: "the atomic problem is
+ * solved in a radial grid ... This produces a series of angular-momentum dependent projectors.  To represent these
+ * projectors in a 3-dimensional grid we need to calculate the spherical harmonics for each point").
+ *
+ * Definition (the paper names the use case but fixes no formula beyond
+ * "radial function times spherical harmonic", so the radial interpolation below is reading #25):
+ *   channel p = 0..nproj-1 has angular momentum l_p and a radial function f_p tabulated on the uniform radial grid
+ *   r_j = j dr, j = 0..nr-1:  radial[p*nr + j] = f_p(r_j).
+ *   f_p(r) = radial[p][j] + (r/dr - j)(radial[p][j+1] - radial[p][j]),  j = floor(r/dr),   for r < (nr-1) dr   (piecewise linear)
+ *   f_p(r) = 0                                                                             for r >= (nr-1) dr  (beyond the table)
+ *   beta_{p,m}(r_vec) = f_p(|r_vec|) R_{l_p}^m(r_vec/|r_vec|),  m = -l_p..l_p                (Eq. 6; r = 0: PAPER.md line 60)
+ *   column of (p, m) = sum_{p' < p} (2 l_{p'} + 1) + (m + l_p);   ncols = sum_p (2 l_p + 1)
+ *   projection:  coeff[v][col] = sum_i w[v][i] beta_col(r_i)       (w = wave-function values times the volume element)
+ * Everything in long double, rounded to double once at the end; the projection is the plain sum in point order.
+ * Parity pins: tests/test_oracle_projector_pins.py (linear-table exactness against the separately pinned R_l^m, table
+ * nodes and midpoints, cutoff, r = 0, column order, quadrature orthonormality of the projection). */
+static ld radial_linear(const double* tab, int nr, ld dr, ld r) {
+    ld t = r / dr;
+    ld fj = floorl(t);
+    if (fj >= (ld)(nr - 1)) return 0.0L;
+    int j = (int)fj;
+    return (ld)tab[j] + (t - fj) * ((ld)tab[j + 1] - (ld)tab[j]);
+}
+
+int sh_oracle_projector_count(int nproj, const int* proj_l) {
+    if (nproj < 0 || (nproj > 0 && !proj_l)) return -1;
+    int ncols = 0;
+    for (int p = 0; p < nproj; ++p) {
+        if (proj_l[p] < 0 || proj_l[p] > LMAX_CAP) return -1;
+        ncols += 2 * proj_l[p] + 1;
+    }
+    return ncols;
+}
+
+/* beta_{p,m} of one point, long double, all columns */
+static void projector_row(const double* p3, int nproj, const int* proj_l, int lmax, const double* radial, int nr, ld dr, ld* row) {
+    ld Yre[KMAX], Yim[KMAX], R[KMAX], mi = 0.0L;
+    ylm_cartesian(lmax, p3[0], p3[1], p3[2], Yre, Yim);
+    real_from_complex(lmax, Yre, Yim, R, &mi);
+    ld x = p3[0], y = p3[1], z = p3[2];
+    ld r = sqrtl(x * x + y * y + z * z);
+    int col = 0;
+    for (int p = 0; p < nproj; ++p) {
+        int l = proj_l[p];
+        ld f = radial_linear(radial + (size_t)p * nr, nr, dr, r);
+        for (int m = -l; m <= l; ++m) row[col++] = f * R[l * (l + 1) + m];
+    }
+}
+
+/* out[i][col], AoS */
+int sh_oracle_projectors(const double* xyz, int64_t n, int nproj, const int* proj_l, const double* radial, int nr, double dr, double* out) {
+    const int ncols = sh_oracle_projector_count(nproj, proj_l);
+    if (ncols < 0 || ncols > KMAX * 4 || n < 0 || nr < 2 || !(dr > 0.0) || (n > 0 && (!xyz || !out || !radial))) return -1;
+    int lmax = 0;
+    for (int p = 0; p < nproj; ++p) if (proj_l[p] > lmax) lmax = proj_l[p];
+    PAR_FOR
+    for (int64_t i = 0; i < n; ++i) {
+        ld row[KMAX * 4];
+        projector_row(xyz + 3 * i, nproj, proj_l, lmax, radial, nr, (ld)dr, row);
+        for (int c = 0; c < ncols; ++c) out[(size_t)i * ncols + c] = (double)row[c];
+    }
+    return 0;
+}
+
+/* coeff[v][col] = sum_i w[v][i] beta_col(r_i): the plain sum, in point order, in long double (single thread).
+ * abs_sum (optional, same shape) receives sum_i |w[v][i] beta_col(r_i)|, the scale of the tolerance. */
+int sh_oracle_project(const double* xyz, int64_t n, int nproj, const int* proj_l, const double* radial, int nr, double dr,
+                      const double* w, int nvec, double* coeff, double* abs_sum) {
+    const int ncols = sh_oracle_projector_count(nproj, proj_l);
+    if (ncols < 0 || ncols > KMAX * 4 || n < 0 || nvec < 0 || nvec > 64 || nr < 2 || !(dr > 0.0)) return -1;
+    if ((n > 0 && (!xyz || !radial || (nvec > 0 && !w))) || (nvec > 0 && !coeff)) return -1;
+    int lmax = 0;
+    for (int p = 0; p < nproj; ++p) if (proj_l[p] > lmax) lmax = proj_l[p];
+    ld* acc = (ld*)calloc((size_t)(nvec > 0 ? nvec : 1) * (ncols > 0 ? ncols : 1) * 2, sizeof(ld));
+    if (!acc) return -2;
+    ld* aabs = acc + (size_t)(nvec > 0 ? nvec : 1) * (ncols > 0 ? ncols : 1);
+    for (int64_t i = 0; i < n; ++i) {
+        ld row[KMAX * 4];
+        projector_row(xyz + 3 * i, nproj, proj_l, lmax, radial, nr, (ld)dr, row);
+        for (int v = 0; v < nvec; ++v) {
+            ld wi = (ld)w[(size_t)v * n + i];
+            for (int c = 0; c < ncols; ++c) {
+                ld term = wi * row[c];
+                acc[(size_t)v * ncols + c] += term;
+                aabs[(size_t)v * ncols + c] += fabsl(term);
+            }
+        }
+    }
+    for (int v = 0; v < nvec; ++v)
+        for (int c = 0; c < ncols; ++c) {
+            coeff[(size_t)v * ncols + c] = (double)acc[(size_t)v * ncols + c];
+            if (abs_sum) abs_sum[(size_t)v * ncols + c] = (double)aabs[(size_t)v * ncols + c];
+        }
+    free(acc);
+    return 0;
+}

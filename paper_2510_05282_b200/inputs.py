@@ -92,3 +92,28 @@ def shard_range(n: int, rank: int, world_size: int) -> tuple[int, int]:
     base, rem = divmod(int(n), world_size)
     begin = rank * base + min(rank, rem)
     return begin, begin + base + (1 if rank < rem else 0)
+
+
+def projector_channels(lmax: int = 3, per_l: int = 2, cutoff: float = 3.0, dr: float = 0.01):
+    """Radial channels of a synthetic norm-conserving-pseudopotential-like projector set ("the atomic
+    problem is solved in a radial grid ... angular-momentum dependent projectors"): `per_l` channels for every l <= lmax,
+    l ascending; channel c of angular momentum l has f(r) = r^l exp(-a_c r^2) (1 - (r/cutoff)^2)^2 for r < cutoff, 0
+    beyond, a_c = 0.8 (c + 1), tabulated at r_j = j dr up to and including the cutoff (last entry exactly 0).
+    Returns (proj_l int32 [nproj], radial float64 [nproj][nr], dr).  No spherical-harmonic arithmetic here."""
+    nr = int(round(cutoff / dr)) + 1
+    r = np.arange(nr, dtype=np.float64) * dr
+    proj_l, rows = [], []
+    for l in range(lmax + 1):
+        for c in range(per_l):
+            f = r**l * np.exp(-0.8 * (c + 1) * r * r) * (1.0 - np.minimum(r / cutoff, 1.0) ** 2) ** 2
+            f[-1] = 0.0
+            proj_l.append(l)
+            rows.append(f)
+    return np.asarray(proj_l, dtype=np.int32), np.ascontiguousarray(np.stack(rows)), float(dr)
+
+
+def wave_weights(n: int, nvec: int = 1, seed: int = 7, volume_element: float = 1.0e-3) -> np.ndarray:
+    """Synthetic projection weights w[v][i] = psi_v(r_i) dV: standard-normal values times the grid's volume element
+    (0.1^3 for the config-2 grid).  Random signs are the hard case for the summation (no smoothness to help)."""
+    rng = np.random.default_rng(seed)
+    return np.ascontiguousarray(rng.standard_normal((nvec, n)) * volume_element)
