@@ -32,7 +32,7 @@
  *
  * Domain: any finite coordinates, including subnormal and huge ones (inputs are pre-scaled by a power
  * of two before r^2 is formed); r = 0 exactly (no epsilon) selects the P:60 convention.  NaN or Inf
- * coordinates give NaN outputs for that point (not an error).
+ * coordinates give NaN in every l >= 1 output of that point (not an error; the l = 0 harmonic is a constant).
  *
  * Errors: every call returns SH_OK (0) or a negative SH_ERR_* code; nothing is thrown and nothing is
  * written on error.  n == 0 is a successful no-op (pointers may then be NULL).
@@ -81,7 +81,8 @@ enum {
     SH_ERR_LMAX = -3,      /* lmax outside [0, 9] */
     SH_ERR_LAYOUT = -4,    /* unknown layout, store-path or front-end bits */
     SH_ERR_ALIGNMENT = -5, /* out not aligned to its element type, or requested store path not possible */
-    SH_ERR_CUDA = -6       /* CUDA launch / copy error; text via sh_last_cuda_error() */
+    SH_ERR_CUDA = -6,      /* CUDA launch / copy error; text via sh_last_cuda_error() */
+    SH_ERR_PROJECTOR = -7  /* sh_projectors / sh_project: nproj, proj_l, nr, dr, nvec or the workspace size is invalid */
 };
 
 /* Real harmonics R_l^m (Eq. 6), fp64.  out: K doubles per point. */
@@ -103,6 +104,37 @@ int sh_real_ext(const double* xyz, int64_t n, int lmax, double* out, int layout,
 int sh_complex_ext(const double* xyz, int64_t n, int lmax, double* out, int layout, void* stream);
 /* Largest lmax the *_ext calls accept (32). */
 int sh_lmax_ext(void);
+
+/* Fused projector consumer (the use case the paper names: "the atomic problem is solved in a radial
+ * grid ... This produces a series of angular-momentum dependent projectors.  To represent these projectors in a
+ * 3-dimensional grid we need to calculate the spherical harmonics for each point").
+ * The harmonics are consumed where they are produced instead of being written out in full:
+ *   channel p = 0..nproj-1 has angular momentum proj_l[p] in [0, 9] and a radial function tabulated on the uniform
+ *   radial grid r_j = j dr:  radial[p*nr + j] = f_p(r_j), j = 0..nr-1 (nr >= 2, dr > 0).  The paper fixes no
+ *   interpolation; this library's reading is piecewise linear,
+ *     f_p(r) = radial[p][j] + (r/dr - j)(radial[p][j+1] - radial[p][j]),  j = floor(r/dr),   for r <  (nr-1) dr
+ *     f_p(r) = 0                                                                             for r >= (nr-1) dr
+ *   (a table should end with 0, as projectors vanish at their cutoff radius, to be continuous there).
+ *   beta_{p,m}(r_vec) = f_p(|r_vec|) R_{l_p}^m(r_vec/|r_vec|), m = -l_p..l_p  (Eq. 6; at r = 0 only l = 0 survives)
+ *   column of (p, m) = sum_{p' < p} (2 proj_l[p'] + 1) + (m + proj_l[p]);  ncols = sh_projector_count(nproj, proj_l).
+ *   NaN or Inf coordinates: every l >= 1 column of that point is NaN, the l = 0 columns are 0 (|r| is not inside the table).
+ * `proj_l` is a HOST array (read during the call); xyz [n][3] Cartesian points relative to the atom, `radial`, `out`,
+ * `w`, `coeff`, `workspace` are DEVICE pointers.  nproj <= SH_MAX_PROJ.  Asynchronous on `stream`; nothing is allocated.
+ *
+ * sh_projectors: out[i*ncols + col] (SH_LAYOUT_AOS) or out[col*n + i] (SH_LAYOUT_SOA) = beta_col(xyz_i); only the
+ *   requested channels are evaluated and written (8 ncols bytes per point instead of 800).
+ * sh_project: coeff[v*ncols + col] = sum_i w[v*n + i] beta_col(xyz_i), v < nvec: the projection <beta|psi> with
+ *   w = psi dV; NOTHING per point is written.  The sum is taken in a fixed order (per-warp partial sums in `workspace`,
+ *   then one ordered pass), so results are reproducible run to run on one device; they differ from the sum in point
+ *   order by rounding only (<= 1e-12 sum_i |w_i beta_i| is the tested bound).  `workspace` must hold at least
+ *   sh_project_workspace_bytes(ncols, nvec) bytes, 8-byte aligned; its contents are scratch. */
+enum { SH_MAX_PROJ = 32 };
+int sh_projector_count(int nproj, const int* proj_l);            /* ncols, or -1 if a proj_l is outside [0, 9] or nproj outside [0, 32] */
+int64_t sh_project_workspace_bytes(int ncols, int nvec);        /* -1 on bad arguments */
+int sh_projectors(const double* xyz, int64_t n, int nproj, const int* proj_l, const double* radial, int nr, double dr,
+                  double* out, int layout, void* stream);
+int sh_project(const double* xyz, int64_t n, int nproj, const int* proj_l, const double* radial, int nr, double dr,
+               const double* w, int nvec, double* coeff, void* workspace, int64_t workspace_bytes, void* stream);
 
 /* Host-buffer entry points: same results, `xyz` and `out` are HOST pointers (pinned memory gives full
  * PCIe speed; pageable memory works).  The call copies chunks host->device, runs the kernels and copies

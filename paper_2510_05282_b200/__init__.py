@@ -14,9 +14,13 @@ from .binding import (  # noqa: F401
     kernel_launch_count,
     load,
     out_shape,
+    project_workspace_bytes,
+    projector_count,
     lmax_ext,
     sh_complex,
     sh_complex_ext,
+    sh_project,
+    sh_projectors,
     sh_real,
     sh_real_ext,
     sh_real_f32,

@@ -72,6 +72,15 @@ def load() -> ctypes.CDLL:
         lib.sh_last_cuda_error.restype = ctypes.c_char_p
         lib.sh_kernel_launch_count.restype = i64
         lib.sh_host_release.restype = None
+        ip = ctypes.POINTER(ci)
+        lib.sh_projector_count.argtypes = [ci, ip]
+        lib.sh_projector_count.restype = ci
+        lib.sh_project_workspace_bytes.argtypes = [ci, ci]
+        lib.sh_project_workspace_bytes.restype = i64
+        lib.sh_projectors.argtypes = [vp, i64, ci, ip, vp, ci, ctypes.c_double, vp, ci, vp]
+        lib.sh_projectors.restype = ci
+        lib.sh_project.argtypes = [vp, i64, ci, ip, vp, ci, ctypes.c_double, vp, ci, vp, vp, i64, vp]
+        lib.sh_project.restype = ci
         _lib = lib
     return _lib
 
@@ -189,3 +198,78 @@ def host_call(kind: str, xyz: "np.ndarray | object", lmax: int, out=None, layout
     if rc != 0:
         raise ShError(rc, f"sh_{kind}_host")
     return ok
+
+
+# ---- fused projector consumer (include/shb200.h "Fused projector consumer") ----
+def _proj_l_array(proj_l):
+    a = (ctypes.c_int * len(proj_l))(*[int(l) for l in proj_l])
+    return a, len(proj_l)
+
+
+def projector_count(proj_l) -> int:
+    """ncols = sum_p (2 l_p + 1); raises if a channel is invalid."""
+    a, k = _proj_l_array(proj_l)
+    c = int(load().sh_projector_count(k, a))
+    if c < 0:
+        raise ShError(-7, "sh_projector_count")
+    return c
+
+
+def project_workspace_bytes(ncols: int, nvec: int) -> int:
+    return int(load().sh_project_workspace_bytes(int(ncols), int(nvec)))
+
+
+def _check_proj_inputs(xyz, radial, nproj):
+    import torch
+
+    if not (xyz.is_cuda and xyz.dtype == torch.float64 and xyz.is_contiguous() and xyz.dim() == 2 and xyz.shape[1] == 3):
+        raise ValueError("xyz must be a contiguous CUDA tensor [n][3] of float64")
+    if not (radial.is_cuda and radial.dtype == torch.float64 and radial.is_contiguous() and radial.dim() == 2 and radial.shape[0] == nproj):
+        raise ValueError("radial must be a contiguous CUDA tensor [nproj][nr] of float64")
+
+
+def sh_projectors(xyz, proj_l, radial, dr, out=None, layout="soa", stream=None):
+    """beta_{p,m}(r_i) = f_p(|r_i|) R_{l_p}^m(r_i/|r_i|) -> AoS [n][ncols] or SoA [ncols][n]; radial [nproj][nr] at r_j = j dr."""
+    import torch
+
+    a, nproj = _proj_l_array(proj_l)
+    _check_proj_inputs(xyz, radial, nproj)
+    n, ncols = xyz.shape[0], projector_count(proj_l)
+    shape = (n, ncols) if _LAYOUTS[layout] == SH_LAYOUT_AOS else (ncols, n)
+    if out is None:
+        out = torch.empty(shape, dtype=torch.float64, device=xyz.device)
+    elif not (out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == n * ncols):
+        raise ValueError(f"out must be a contiguous CUDA float64 tensor with {n * ncols} elements")
+    s = torch.cuda.current_stream(xyz.device).cuda_stream if stream is None else int(stream)
+    with torch.cuda.device(xyz.device):
+        rc = load().sh_projectors(xyz.data_ptr(), n, nproj, a, radial.data_ptr(), radial.shape[1], float(dr), out.data_ptr(), _LAYOUTS[layout], s)
+    if rc != 0:
+        raise ShError(rc, "sh_projectors")
+    return out
+
+
+def sh_project(xyz, proj_l, radial, dr, w, coeff=None, workspace=None, stream=None):
+    """coeff[v][col] = sum_i w[v][i] beta_col(r_i); w [nvec][n] CUDA float64 -> coeff [nvec][ncols].  `workspace` (a CUDA
+    uint8 tensor of at least project_workspace_bytes(ncols, nvec) bytes) is allocated with PyTorch when not given."""
+    import torch
+
+    a, nproj = _proj_l_array(proj_l)
+    _check_proj_inputs(xyz, radial, nproj)
+    n, ncols = xyz.shape[0], projector_count(proj_l)
+    if not (w.is_cuda and w.dtype == torch.float64 and w.is_contiguous() and w.dim() == 2 and w.shape[1] == n):
+        raise ValueError("w must be a contiguous CUDA tensor [nvec][n] of float64")
+    nvec = w.shape[0]
+    if coeff is None:
+        coeff = torch.empty((nvec, ncols), dtype=torch.float64, device=xyz.device)
+    elif not (coeff.is_cuda and coeff.dtype == torch.float64 and coeff.is_contiguous() and coeff.numel() == nvec * ncols):
+        raise ValueError(f"coeff must be a contiguous CUDA float64 tensor with {nvec * ncols} elements")
+    need = project_workspace_bytes(ncols, nvec)
+    if workspace is None:
+        workspace = torch.empty(max(need, 8), dtype=torch.uint8, device=xyz.device)
+    s = torch.cuda.current_stream(xyz.device).cuda_stream if stream is None else int(stream)
+    with torch.cuda.device(xyz.device):
+        rc = load().sh_project(xyz.data_ptr(), n, nproj, a, radial.data_ptr(), radial.shape[1], float(dr), w.data_ptr(), nvec,
+                               coeff.data_ptr(), workspace.data_ptr(), workspace.numel() * workspace.element_size(), s)
+    if rc != 0:
+        raise ShError(rc, "sh_project")
+    return coeff

@@ -710,6 +710,288 @@ __global__ void __launch_bounds__(WARPS * 32) sh_aos_kernel(const TI* __restrict
 }
 
 // ------------------------------------------------------------------------------------------------
+// Fused projector consumer (the use case of P:14; include/shb200.h "Fused projector
+// consumer"): beta_{p,m}(r_vec) = f_p(|r_vec|) R_{l_p}^m(r_vec/|r_vec|) with f_p piecewise linear on a uniform radial grid.
+// The l-blocks are produced as above (a3-a5) and consumed in registers: each block is scaled by the radial value of
+// every channel of that l and either stored (sh_projectors: only the requested columns, 8 ncols B/point) or contracted
+// with the weight vectors (sh_project: nothing per point is written -- the path is then bound by the FP64 pipe).
+// l-blocks no channel asks for are skipped by a warp-uniform branch.
+struct ProjPlan {
+    int ncols;                             // columns of this launch
+    int nr;                                // radial table length
+    double inv_dr;
+    unsigned char first[shgen::LMAX_CAP + 2];   // channel slots of block l: [first[l], first[l+1])  (slots sorted by l)
+    unsigned char chan[SH_MAX_PROJ];       // slot -> row of `radial`
+    unsigned short col[SH_MAX_PROJ];       // slot -> first column of the channel in this launch's output
+};
+
+// position of |r| in the radial table: j = floor(r/dr), u = r/dr - j; beyond the table (and for NaN) `in` is false
+struct RadialPos {
+    int j;
+    double u;
+    bool in;
+    __device__ __forceinline__ RadialPos(double x, double y, double z, const ProjPlan& plan) {
+        const double r = sqrt(x * x + y * y + z * z);   // unscaled: 0 for r < 1e-162 (table start), +Inf beyond 1e154 (past any table)
+        const double t = r * plan.inv_dr;
+        in = t < (double)(plan.nr - 1);
+        j = in ? (int)t : 0;
+        u = in ? t - (double)j : 0.0;
+    }
+    __device__ __forceinline__ double f(const double* __restrict__ radial, int nr, int channel) const {
+        const double* tab = radial + (int64_t)channel * nr + j;
+        const double a = __ldg(tab), b = __ldg(tab + 1);
+        return in ? fma(u, b - a, a) : 0.0;
+    }
+};
+
+// the real harmonics of block l in ascending m (a3-a5), handed to the sink one block at a time
+template <int LMAX, class Sink>
+__device__ __forceinline__ void eval_projector_blocks(const UnitVec& u, const ProjPlan& plan, Sink& sink) {
+    const Azim<LMAX, double> az(u.x, u.y);
+    static_for<0, LMAX + 1>([&](auto lc) {
+        constexpr int L = decltype(lc)::value;
+        if (plan.first[L] != plan.first[L + 1]) {
+            double blk[2 * L + 1];
+            static_for<0, L + 1>([&](auto mc) {
+                constexpr int M = decltype(mc)::value;
+                constexpr double A = shgen::A_REAL[L][M];
+                double q = A * shgen::Polar<L, M, double>::eval(u.z);
+                if constexpr (M == 0) {
+                    if constexpr (L > 0 && L % 2 == 0) q = zero_where(u.origin, q);   // P_l(0) != 0: the r = 0 convention needs it
+                    blk[L] = q;
+                } else {
+                    blk[L - M] = q * az.S[M];
+                    blk[L + M] = q * az.C[M];
+                }
+            });
+            sink.template block<L>(blk);
+        }
+    });
+}
+
+struct ProjSoASink {
+    double* p;         // out + i
+    int64_t n;
+    const double* radial;
+    const ProjPlan& plan;
+    const RadialPos& pos;
+    template <int L> __device__ __forceinline__ void block(const double (&blk)[2 * L + 1]) {
+        for (int s = plan.first[L]; s < plan.first[L + 1]; ++s) {
+            const double f = pos.f(radial, plan.nr, plan.chan[s]);
+            double* q = p + (int64_t)plan.col[s] * n;
+            static_for<0, 2 * L + 1>([&](auto mc) { __stcs(q + decltype(mc)::value * n, f * blk[decltype(mc)::value]); });
+        }
+    }
+};
+
+template <int LMAX>
+__global__ void __launch_bounds__(256) sh_proj_soa_kernel(const double* __restrict__ xyz, int64_t n, const double* __restrict__ radial,
+                                                           const __grid_constant__ ProjPlan plan, double* __restrict__ out, InputPrefetch pf) {
+    prefetch_input_window(xyz, n * 24, (int64_t)256 * 24, pf);
+    const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (i >= n) return;
+    RawPoint<double> pt;
+    pt.load(xyz, i);
+    const RadialPos pos(pt.x, pt.y, pt.z, plan);
+    ProjSoASink sink{out + i, n, radial, plan, pos};
+    eval_projector_blocks<LMAX>(pt.unit(SH_COORDS_CARTESIAN), plan, sink);
+}
+
+// sh_projectors, AoS: one warp = one 32-point tile.  Each lane stages its point's row in the warp's shared-memory tile
+// (pitch odd: conflict-free 8-byte stores); the tile is one contiguous span of `out`, copied out by the warp with coalesced
+// streaming stores.
+struct ProjRowSink {
+    double* row;
+    const double* radial;
+    const ProjPlan& plan;
+    const RadialPos& pos;
+    template <int L> __device__ __forceinline__ void block(const double (&blk)[2 * L + 1]) {
+        for (int s = plan.first[L]; s < plan.first[L + 1]; ++s) {
+            const double f = pos.f(radial, plan.nr, plan.chan[s]);
+            double* q = row + plan.col[s];
+            static_for<0, 2 * L + 1>([&](auto mc) { q[decltype(mc)::value] = f * blk[decltype(mc)::value]; });
+        }
+    }
+};
+
+template <int LMAX>
+__global__ void __launch_bounds__(128) sh_proj_aos_kernel(const double* __restrict__ xyz, int64_t n, const double* __restrict__ radial,
+                                                           const __grid_constant__ ProjPlan plan, double* __restrict__ out, InputPrefetch pf) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, warps = blockDim.x >> 5;
+    prefetch_input_window(xyz, n * 24, (int64_t)warps * 32 * 24, pf);
+    const int ncols = plan.ncols, pitch = ncols | 1;
+    double* tile = reinterpret_cast<double*>(smem_raw) + (size_t)warp * 32 * pitch;
+    const int64_t base = ((int64_t)blockIdx.x * warps + warp) << 5;
+    if (base >= n) return;
+    const int64_t i = base + lane;
+    const int rows = (n - base) < 32 ? (int)(n - base) : 32;
+    if (i < n) {
+        RawPoint<double> pt;
+        pt.load(xyz, i);
+        const RadialPos pos(pt.x, pt.y, pt.z, plan);
+        ProjRowSink sink{tile + lane * pitch, radial, plan, pos};
+        eval_projector_blocks<LMAX>(pt.unit(SH_COORDS_CARTESIAN), plan, sink);
+    }
+    __syncwarp();
+    double* g = out + base * ncols;
+    const int total = rows * ncols;
+    int r = 0, c = lane;
+    while (c >= ncols) { c -= ncols; ++r; }
+    for (int e = lane; e < total; e += 32) {
+        __stcs(g + e, tile[r * pitch + c]);
+        c += 32;
+        while (c >= ncols) { c -= ncols; ++r; }
+    }
+}
+
+// sh_project: coeff[v][col] = sum_i w[v][i] beta_col(r_i).  Nothing per point is written, so the FP64 pipe is the bound.
+// One warp = one 32-point tile at a time, tiles dealt round-robin over all warps of a grid that fills the machine once;
+// the next tile's point and weights are loaded before the current tile is evaluated.  The l-blocks a lane produces are
+// staged, scaled by the radial values, in SEGMENTS of at most 32 columns (whole channels, packed in the order of
+// production; segment plan in ProjSegments) in the warp's [32][33] shared-memory tile; when a segment is complete, lane c
+// sums column c over the tile's rows against the tile's weights (32 conflict-free loads and FMAs per weight vector)
+// and adds the result to the warp's running sums in shared memory.  Running sums are kept in the order of production
+// ("slot order"); every warp writes them to `partial` [warp][nvec][ncols] at the end, and sh_project_reduce_kernel adds
+// the warps in a fixed order and scatters to the caller's column order.
+constexpr int PROJ_NV = 4;          // weight vectors contracted per launch
+constexpr int PROJ_MAX_COLS = 128;  // columns per launch (whole channels); wider channel lists run as several launches
+constexpr int PROJ_SEG_PITCH = 33;
+constexpr int PROJECT_SMEM_DOUBLES_PER_WARP = 32 * PROJ_SEG_PITCH + PROJ_NV * PROJ_MAX_COLS + PROJ_NV * 32;   // tile, running sums, weights
+
+struct ProjSegments {
+    unsigned short scol[SH_MAX_PROJ];   // slot -> its first column in slot order
+    unsigned short sbeg[SH_MAX_PROJ];   // slot -> first column (slot order) of the segment the slot belongs to
+    unsigned char flush[SH_MAX_PROJ];   // slot -> 1 if the segment is complete after this slot
+};
+
+struct ProjectSink {
+    double* tile;        // the warp's [32][PROJ_SEG_PITCH] segment tile
+    double* sums;        // the warp's running sums [PROJ_NV][PROJ_MAX_COLS]
+    const double* wt;    // the tile's weights [PROJ_NV][32]
+    const double* radial;
+    const ProjPlan& plan;
+    const ProjSegments& seg;
+    const RadialPos& pos;
+    int lane, rows, nvec;
+
+    __device__ __forceinline__ void flush(int begin, int len) {
+        __syncwarp();
+        if (lane < len) {
+            static_for<0, PROJ_NV>([&](auto vc) {
+                constexpr int V = decltype(vc)::value;
+                if (V < nvec) {
+                    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;   // four chains: the FMA latency is not the limit
+                    const double* t = tile + lane;
+                    const double* wv = wt + V * 32;
+                    if (rows == 32) {
+#pragma unroll
+                        for (int r = 0; r < 32; r += 4) {
+                            s0 = fma(t[(r + 0) * PROJ_SEG_PITCH], wv[r + 0], s0);
+                            s1 = fma(t[(r + 1) * PROJ_SEG_PITCH], wv[r + 1], s1);
+                            s2 = fma(t[(r + 2) * PROJ_SEG_PITCH], wv[r + 2], s2);
+                            s3 = fma(t[(r + 3) * PROJ_SEG_PITCH], wv[r + 3], s3);
+                        }
+                    } else {
+                        for (int r = 0; r < rows; ++r) s0 = fma(t[r * PROJ_SEG_PITCH], wv[r], s0);
+                    }
+                    sums[V * PROJ_MAX_COLS + begin + lane] += (s0 + s1) + (s2 + s3);
+                }
+            });
+        }
+        __syncwarp();
+    }
+
+    template <int L> __device__ __forceinline__ void block(const double (&blk)[2 * L + 1]) {
+        for (int s = plan.first[L]; s < plan.first[L + 1]; ++s) {
+            const double f = pos.f(radial, plan.nr, plan.chan[s]);
+            const int c0 = seg.scol[s], b0 = seg.sbeg[s];
+            double* q = tile + lane * PROJ_SEG_PITCH + (c0 - b0);
+            static_for<0, 2 * L + 1>([&](auto mc) { q[decltype(mc)::value] = f * blk[decltype(mc)::value]; });
+            if (seg.flush[s]) flush(b0, c0 + 2 * L + 1 - b0);
+        }
+    }
+};
+
+template <int LMAX>
+__global__ void __launch_bounds__(128, 3) sh_project_kernel(const double* __restrict__ xyz, int64_t n, const double* __restrict__ radial,
+                                                             const __grid_constant__ ProjPlan plan, const __grid_constant__ ProjSegments seg,
+                                                             const double* __restrict__ w, int nvec, double* __restrict__ partial) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double* s_tile = reinterpret_cast<double*>(smem_raw) + (size_t)warp * PROJECT_SMEM_DOUBLES_PER_WARP;
+    double* s_sums = s_tile + 32 * PROJ_SEG_PITCH;
+    double* s_wt = s_sums + PROJ_NV * PROJ_MAX_COLS;
+    const int ncols = plan.ncols;
+    for (int e = lane; e < PROJ_NV * PROJ_MAX_COLS; e += 32) s_sums[e] = 0.0;
+    const int64_t ntiles = (n + 31) >> 5;
+    const int64_t gw = (int64_t)blockIdx.x * 4 + warp, nw = (int64_t)gridDim.x * 4;
+    // every lane takes part in the warp-level segment sums, so idle lanes of the last tile evaluate a clamped point
+    // (their rows are not summed)
+    auto point_of = [&](int64_t t) { const int64_t i = (t << 5) + lane; return i < n ? i : n - 1; };
+    RawPoint<double> cur, nxt;
+    double wc[PROJ_NV], wn[PROJ_NV];
+    auto load = [&](int64_t t, RawPoint<double>& pt, double (&wv)[PROJ_NV]) {
+        const int64_t i = point_of(t);
+        pt.load(xyz, i);
+        static_for<0, PROJ_NV>([&](auto vc) {
+            constexpr int V = decltype(vc)::value;
+            wv[V] = V < nvec ? __ldg(w + (int64_t)V * n + i) : 0.0;
+        });
+    };
+    int64_t t = gw;
+    if (t < ntiles) load(t, cur, wc);
+    for (; t < ntiles; t += nw) {
+        const bool have_next = t + nw < ntiles;
+        if (have_next) load(t + nw, nxt, wn);
+        const int64_t left = n - (t << 5);
+        static_for<0, PROJ_NV>([&](auto vc) { s_wt[decltype(vc)::value * 32 + lane] = wc[decltype(vc)::value]; });
+        const RadialPos pos(cur.x, cur.y, cur.z, plan);
+        ProjectSink sink{s_tile, s_sums, s_wt, radial, plan, seg, pos, lane, left < 32 ? (int)left : 32, nvec};
+        eval_projector_blocks<LMAX>(cur.unit(SH_COORDS_CARTESIAN), plan, sink);
+        cur = nxt;
+        static_for<0, PROJ_NV>([&](auto vc) { wc[decltype(vc)::value] = wn[decltype(vc)::value]; });
+    }
+    __syncwarp();
+    for (int v = 0; v < nvec; ++v)
+        for (int c = lane; c < ncols; c += 32) partial[(gw * nvec + v) * ncols + c] = s_sums[v * PROJ_MAX_COLS + c];
+}
+
+// coeff[v*coeff_stride + user column] = sum over warps of partial[warp][v][slot-order column], the warps added in a fixed
+// order (reproducible): 32 lanes = 32 consecutive (v, column) elements; the block's 16 warps each add every 16th warp of
+// `partial` (coalesced, four loads in flight), then the 16 sums are added in order.
+__global__ void __launch_bounds__(512) sh_project_reduce_kernel(const double* __restrict__ partial, int nwarps, int nvec, const __grid_constant__ ProjPlan plan,
+                                                                 const __grid_constant__ ProjSegments seg, double* __restrict__ coeff, int coeff_stride) {
+    __shared__ double s[16][32];
+    const int ncols = plan.ncols, ne = nvec * ncols;
+    const int y = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int e = blockIdx.x * 32 + lane;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    if (e < ne) {
+        int g = y;
+        for (; g + 48 < nwarps; g += 64) {
+            a0 += partial[(int64_t)g * ne + e];
+            a1 += partial[(int64_t)(g + 16) * ne + e];
+            a2 += partial[(int64_t)(g + 32) * ne + e];
+            a3 += partial[(int64_t)(g + 48) * ne + e];
+        }
+        for (; g < nwarps; g += 16) a0 += partial[(int64_t)g * ne + e];
+    }
+    s[y][lane] = (a0 + a1) + (a2 + a3);
+    __syncthreads();
+    if (y == 0 && e < ne) {
+        double t = 0.0;
+        for (int k = 0; k < 16; ++k) t += s[k][lane];
+        // slot-order column -> the caller's column
+        const int v = e / ncols, c = e - v * ncols;
+        int slot = 0;
+        const int nslots = plan.first[shgen::LMAX_CAP + 1];
+        while (slot + 1 < nslots && seg.scol[slot + 1] <= c) ++slot;
+        coeff[v * coeff_stride + plan.col[slot] + (c - seg.scol[slot])] = t;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // host side
 std::atomic<int64_t> g_launches{0};
 thread_local char g_cuda_error[256] = "";
@@ -1010,6 +1292,195 @@ int run_host(const TI* xyz, int64_t n, int lmax, T* out, int layout_bits) {
     return rc;
 }
 
+// ---- fused projector consumer, host side ----
+// ncols of a channel list, or -1
+int projector_count(int nproj, const int* proj_l) {
+    if (nproj < 0 || nproj > SH_MAX_PROJ || (nproj > 0 && !proj_l)) return -1;
+    int ncols = 0;
+    for (int p = 0; p < nproj; ++p) {
+        if (proj_l[p] < 0 || proj_l[p] > shgen::LMAX_CAP) return -1;
+        ncols += 2 * proj_l[p] + 1;
+    }
+    return ncols;
+}
+
+// plan for the channels [p0, p1): slots sorted by l, columns relative to the first column of channel p0; returns the largest l
+int make_plan(const int* proj_l, int p0, int p1, int nr, double dr, ProjPlan& plan) {
+    std::memset(&plan, 0, sizeof(plan));
+    plan.nr = nr;
+    plan.inv_dr = 1.0 / dr;
+    int col0[SH_MAX_PROJ], ncols = 0, lmax = 0;
+    for (int p = p0; p < p1; ++p) {
+        col0[p] = ncols;
+        ncols += 2 * proj_l[p] + 1;
+        if (proj_l[p] > lmax) lmax = proj_l[p];
+    }
+    plan.ncols = ncols;
+    int slot = 0;
+    for (int l = 0; l <= shgen::LMAX_CAP; ++l) {
+        plan.first[l] = (unsigned char)slot;
+        for (int p = p0; p < p1; ++p)
+            if (proj_l[p] == l) {
+                plan.chan[slot] = (unsigned char)p;
+                plan.col[slot] = (unsigned short)col0[p];
+                ++slot;
+            }
+    }
+    plan.first[shgen::LMAX_CAP + 1] = (unsigned char)slot;
+    return lmax;
+}
+
+int check_projector_args(const double* xyz, int64_t n, int nproj, const int* proj_l, const double* radial, int nr, double dr) {
+    if (n < 0) return SH_ERR_COUNT;
+    if (projector_count(nproj, proj_l) < 0 || nr < 2 || !(dr > 0.0) || !(1.0 / dr > 0.0) || !(1.0 / dr <= DBL_MAX)) return SH_ERR_PROJECTOR;
+    if (n > 0 && (!xyz || (nproj > 0 && !radial))) return SH_ERR_NULL;
+    if (!aligned(xyz, 8) || !aligned(radial, 8)) return SH_ERR_ALIGNMENT;
+    return SH_OK;
+}
+
+constexpr int PROJ_CTAS_PER_SM = 3;   // grid of sh_project_kernel: the machine filled once (what the workspace is sized for)
+
+template <int LMAX>
+int launch_proj_aos(const double* xyz, int64_t n, const double* radial, const ProjPlan& plan, double* out, cudaStream_t st) {
+    auto kern = sh_proj_aos_kernel<LMAX>;
+    const size_t per_warp = (size_t)32 * (plan.ncols | 1) * sizeof(double);
+    int warps = 4;
+    while (warps > 1 && warps * per_warp > (size_t)56 * 1024) warps >>= 1;   // four CTAs per SM while the row width allows it
+    const size_t smem = warps * per_warp;
+    if (smem > (size_t)227 * 1024) return SH_ERR_PROJECTOR;
+    static size_t smem_set = 0;   // the opt-in limit only ever grows
+    if (smem > 48 * 1024 && smem > smem_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return cuda_fail(e);
+        smem_set = smem;
+    }
+    const int64_t ntiles = (n + 31) / 32;
+    const int64_t blocks = (ntiles + warps - 1) / warps;
+    if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
+    kern<<<(unsigned)blocks, warps * 32, smem, st>>>(xyz, n, radial, plan, out, prefetch_plan(n, (int64_t)warps * 32));
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? SH_OK : cuda_fail(e);
+}
+
+template <int LMAX>
+int launch_proj_soa(const double* xyz, int64_t n, const double* radial, const ProjPlan& plan, double* out, cudaStream_t st) {
+    const int64_t blocks = (n + 255) / 256;
+    if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
+    sh_proj_soa_kernel<LMAX><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, radial, plan, out, prefetch_plan(n, 256));
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? SH_OK : cuda_fail(e);
+}
+
+int run_projectors(const double* xyz, int64_t n, int nproj, const int* proj_l, const double* radial, int nr, double dr, double* out,
+                   int layout_bits, void* stream) {
+    int rc = check_projector_args(xyz, n, nproj, proj_l, radial, nr, dr);
+    if (rc != SH_OK) return rc;
+    if (layout_bits != SH_LAYOUT_AOS && layout_bits != SH_LAYOUT_SOA) return SH_ERR_LAYOUT;   // Cartesian points, automatic store path
+    if (n == 0 || nproj == 0) return SH_OK;
+    if (!out) return SH_ERR_NULL;
+    if (!aligned(out, 8)) return SH_ERR_ALIGNMENT;
+    ProjPlan plan;
+    const int lmax = make_plan(proj_l, 0, nproj, nr, dr, plan);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    switch (lmax) {
+#define SH_CASE(L) case L: return layout_bits == SH_LAYOUT_SOA ? launch_proj_soa<L>(xyz, n, radial, plan, out, st) \
+                                                             : launch_proj_aos<L>(xyz, n, radial, plan, out, st);
+        SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(3) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8) SH_CASE(9)
+#undef SH_CASE
+    }
+    return SH_ERR_PROJECTOR;
+}
+
+// segments of at most 32 columns, whole channels, packed greedily in slot order (the order of production)
+void make_segments(const int* proj_l, const ProjPlan& plan, ProjSegments& seg) {
+    std::memset(&seg, 0, sizeof(seg));
+    const int nslots = plan.first[shgen::LMAX_CAP + 1];
+    int col = 0, beg = 0;
+    for (int s = 0; s < nslots; ++s) {
+        const int len = 2 * proj_l[plan.chan[s]] + 1;
+        if (col + len - beg > 32) {
+            seg.flush[s - 1] = 1;
+            beg = col;
+        }
+        seg.scol[s] = (unsigned short)col;
+        seg.sbeg[s] = (unsigned short)beg;
+        col += len;
+    }
+    if (nslots > 0) seg.flush[nslots - 1] = 1;
+}
+
+int64_t project_workspace_bytes(int ncols, int nvec) {
+    if (ncols < 0 || nvec < 0) return -1;
+    const int64_t cols = ncols < PROJ_MAX_COLS ? ncols : PROJ_MAX_COLS, vecs = nvec < PROJ_NV ? nvec : PROJ_NV;
+    return (int64_t)sm_count() * PROJ_CTAS_PER_SM * 4 * vecs * cols * (int64_t)sizeof(double);
+}
+
+template <int LMAX>
+int launch_project(const double* xyz, int64_t n, const double* radial, const ProjPlan& plan, const ProjSegments& seg, const double* w, int nvec,
+                   double* partial, double* coeff, int coeff_stride, cudaStream_t st) {
+    const int64_t ntiles = (n + 31) / 32;
+    int64_t blocks = (ntiles + 3) / 4;
+    const int64_t cap = (int64_t)sm_count() * PROJ_CTAS_PER_SM;
+    if (blocks > cap) blocks = cap;
+    constexpr size_t smem = (size_t)4 * PROJECT_SMEM_DOUBLES_PER_WARP * sizeof(double);   // 53 KB: above the 48 KB default
+    static bool opted_in = false;
+    if (!opted_in) {
+        cudaError_t e = cudaFuncSetAttribute(sh_project_kernel<LMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return cuda_fail(e);
+        opted_in = true;
+    }
+    sh_project_kernel<LMAX><<<(unsigned)blocks, 128, smem, st>>>(xyz, n, radial, plan, seg, w, nvec, partial);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e);
+    const int elems = nvec * plan.ncols;
+    sh_project_reduce_kernel<<<(elems + 31) / 32, 512, 0, st>>>(partial, (int)blocks * 4, nvec, plan, seg, coeff, coeff_stride);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    e = cudaGetLastError();
+    return e == cudaSuccess ? SH_OK : cuda_fail(e);
+}
+
+int run_project(const double* xyz, int64_t n, int nproj, const int* proj_l, const double* radial, int nr, double dr, const double* w,
+                int nvec, double* coeff, void* workspace, int64_t workspace_bytes, void* stream) {
+    int rc = check_projector_args(xyz, n, nproj, proj_l, radial, nr, dr);
+    if (rc != SH_OK) return rc;
+    if (nvec < 0) return SH_ERR_PROJECTOR;
+    const int ncols = projector_count(nproj, proj_l);
+    if (nvec == 0 || ncols == 0) return SH_OK;
+    if (!coeff || (n > 0 && !w)) return SH_ERR_NULL;
+    if (!aligned(coeff, 8) || !aligned(w, 8) || !aligned(workspace, 8)) return SH_ERR_ALIGNMENT;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (n == 0) {   // the empty sum
+        cudaError_t e = cudaMemsetAsync(coeff, 0, (size_t)nvec * ncols * sizeof(double), st);
+        return e == cudaSuccess ? SH_OK : cuda_fail(e);
+    }
+    if (!workspace || workspace_bytes < project_workspace_bytes(ncols, nvec)) return SH_ERR_PROJECTOR;
+    double* partial = static_cast<double*>(workspace);
+    // a launch covers at most PROJ_MAX_COLS columns (whole channels) and PROJ_NV weight vectors; the workspace is reused in stream order
+    for (int p0 = 0, c0 = 0; p0 < nproj;) {
+        int p1 = p0, cols = 0;
+        while (p1 < nproj && cols + 2 * proj_l[p1] + 1 <= PROJ_MAX_COLS) cols += 2 * proj_l[p1++] + 1;
+        ProjPlan plan;
+        ProjSegments seg;
+        const int lmax = make_plan(proj_l, p0, p1, nr, dr, plan);
+        make_segments(proj_l, plan, seg);
+        for (int v0 = 0; v0 < nvec; v0 += PROJ_NV) {
+            const int nv = nvec - v0 < PROJ_NV ? nvec - v0 : PROJ_NV;
+            switch (lmax) {
+#define SH_CASE(L) case L: rc = launch_project<L>(xyz, n, radial, plan, seg, w + (int64_t)v0 * n, nv, partial, coeff + (int64_t)v0 * ncols + c0, ncols, st); break;
+                SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(3) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8) SH_CASE(9)
+#undef SH_CASE
+            }
+            if (rc != SH_OK) return rc;
+        }
+        p0 = p1;
+        c0 += cols;
+    }
+    return SH_OK;
+}
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------------------
@@ -1035,6 +1506,17 @@ int sh_complex_ext(const double* xyz, int64_t n, int lmax, double* out, int layo
     return run_device_ext<KIND_COMPLEX>(xyz, n, lmax, out, layout, stream);
 }
 int sh_lmax_ext(void) { return shgen::LMAX_EXT; }
+
+int sh_projector_count(int nproj, const int* proj_l) { return projector_count(nproj, proj_l); }
+int64_t sh_project_workspace_bytes(int ncols, int nvec) { return project_workspace_bytes(ncols, nvec); }
+int sh_projectors(const double* xyz, int64_t n, int nproj, const int* proj_l, const double* radial, int nr, double dr, double* out,
+                  int layout, void* stream) {
+    return run_projectors(xyz, n, nproj, proj_l, radial, nr, dr, out, layout, stream);
+}
+int sh_project(const double* xyz, int64_t n, int nproj, const int* proj_l, const double* radial, int nr, double dr, const double* w,
+               int nvec, double* coeff, void* workspace, int64_t workspace_bytes, void* stream) {
+    return run_project(xyz, n, nproj, proj_l, radial, nr, dr, w, nvec, coeff, workspace, workspace_bytes, stream);
+}
 
 int sh_real_host(const double* xyz, int64_t n, int lmax, double* out, int layout) {
     return run_host<KIND_REAL, double, double>(xyz, n, lmax, out, layout);
@@ -1081,6 +1563,7 @@ const char* sh_strerror(int code) {
         case SH_ERR_LAYOUT: return "unknown layout, store-path or front-end bits, or a layout this call does not offer";
         case SH_ERR_ALIGNMENT: return "pointer not aligned to its element type, or requested store path impossible for this alignment";
         case SH_ERR_CUDA: return "CUDA error (see sh_last_cuda_error)";
+        case SH_ERR_PROJECTOR: return "bad projector arguments (nproj, proj_l, nr, dr, nvec or workspace size)";
     }
     return "unknown error code";
 }

@@ -75,7 +75,31 @@ def test_argument_validation_without_gpu(lib):
         assert fn(p, 4, 20, p + 4, 1, None) == -5
     for fn in (lib.sh_real_host, lib.sh_complex_host, lib.sh_spinor_host, lib.sh_real_f32_host):
         assert fn(p, -1, 3, p, 0) == -2 and fn(p, 1, 11, p, 0) == -3 and fn(None, 0, 3, None, 1) == 0
-    for code in range(-6, 1):
+    # fused projector consumer: every argument is checked on the host
+    ip = ctypes.POINTER(ctypes.c_int)
+    ls = (ctypes.c_int * 3)(0, 1, 2)
+    bad = (ctypes.c_int * 2)(0, 10)
+    assert lib.sh_projector_count(3, ls) == 9 and lib.sh_projector_count(0, None) == 0
+    assert lib.sh_projector_count(2, bad) == -1 and lib.sh_projector_count(33, ls) == -1 and lib.sh_projector_count(-1, ls) == -1
+    assert lib.sh_project_workspace_bytes(-1, 1) == -1 and lib.sh_project_workspace_bytes(9, -1) == -1
+    assert lib.sh_projectors(p, -1, 3, ls, p, 8, 0.1, p, 1, None) == -2          # n < 0
+    assert lib.sh_projectors(p, 4, 2, bad, p, 8, 0.1, p, 1, None) == -7          # l = 10
+    assert lib.sh_projectors(p, 4, 3, ls, p, 1, 0.1, p, 1, None) == -7           # nr < 2
+    assert lib.sh_projectors(p, 4, 3, ls, p, 8, 0.0, p, 1, None) == -7           # dr <= 0
+    assert lib.sh_projectors(p, 4, 3, ls, p, 8, float("nan"), p, 1, None) == -7
+    assert lib.sh_projectors(None, 4, 3, ls, p, 8, 0.1, p, 1, None) == -1
+    assert lib.sh_projectors(p, 4, 3, ls, None, 8, 0.1, p, 1, None) == -1
+    assert lib.sh_projectors(p, 4, 3, ls, p, 8, 0.1, None, 1, None) == -1
+    assert lib.sh_projectors(p, 4, 3, ls, p, 8, 0.1, p, 2, None) == -4           # layout
+    assert lib.sh_projectors(p, 4, 3, ls, p, 8, 0.1, p, 1 | (1 << 16), None) == -4  # Cartesian points only
+    assert lib.sh_projectors(p, 4, 3, ls, p, 8, 0.1, p + 4, 1, None) == -5
+    assert lib.sh_projectors(None, 0, 3, ls, None, 8, 0.1, None, 0, None) == 0   # n = 0
+    assert lib.sh_project(p, -1, 3, ls, p, 8, 0.1, p, 1, p, p, 1 << 30, None) == -2
+    assert lib.sh_project(p, 4, 3, ls, p, 8, 0.1, p, -1, p, p, 1 << 30, None) == -7
+    assert lib.sh_project(p, 4, 3, ls, p, 8, 0.1, None, 1, p, p, 1 << 30, None) == -1
+    assert lib.sh_project(p, 4, 3, ls, p, 8, 0.1, p, 1, None, p, 1 << 30, None) == -1
+    assert lib.sh_project(p, 4, 3, ls, p, 8, 0.1, p, 0, None, None, 0, None) == 0  # nvec = 0
+    for code in range(-7, 1):
         assert len(lib.sh_strerror(code)) > 1
     assert lib.sh_strerror(-99) == b"unknown error code"
 
