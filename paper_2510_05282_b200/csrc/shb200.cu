@@ -849,15 +849,22 @@ __global__ void __launch_bounds__(128) sh_proj_aos_kernel(const double* __restri
 // One warp = one 32-point tile at a time, tiles dealt round-robin over all warps of a grid that fills the machine once;
 // the next tile's point and weights are loaded before the current tile is evaluated.  The l-blocks a lane produces are
 // staged, scaled by the radial values, in SEGMENTS of at most 32 columns (whole channels, packed in the order of
-// production; segment plan in ProjSegments) in the warp's [32][33] shared-memory tile; when a segment is complete, lane c
-// sums column c over the tile's rows against the tile's weights (32 conflict-free loads and FMAs per weight vector)
-// and adds the result to the warp's running sums in shared memory.  Running sums are kept in the order of production
-// ("slot order"); every warp writes them to `partial` [warp][nvec][ncols] at the end, and sh_project_reduce_kernel adds
-// the warps in a fixed order and scatters to the caller's column order.
+// production; segment plan in ProjSegments) in the warp's shared-memory tile, TRANSPOSED: tile[column][point], pitch 34
+// doubles, so a lane's staging stores are conflict-free 8-byte stores (32 consecutive doubles per column) and, when a
+// segment is complete, lane c sums column c over the 32 points with 16-byte loads (rows 272 B apart: eight lanes per
+// 128-byte wavefront, conflict-free) and adds the result to the warp's running sums in shared memory.
+//   NV = 1: the weight is folded into the radial value (beta w is staged), the column sum is 32 additions;
+//   NV = 4: up to four weight vectors; the tile's weights sit in shared memory as [point][4] and are read as broadcasts.
+// Idle lanes of a ragged last tile evaluate the point (0, 0, 1) with weight 0, so every column sum runs over 32 rows.
+// Running sums are kept in the order of production ("slot order"); every warp writes them to `partial`
+// [warp][nvec][ncols] at the end, and sh_project_reduce_kernel adds the warps in a fixed order and scatters to the
+// caller's column order.
 constexpr int PROJ_NV = 4;          // weight vectors contracted per launch
 constexpr int PROJ_MAX_COLS = 128;  // columns per launch (whole channels); wider channel lists run as several launches
-constexpr int PROJ_SEG_PITCH = 33;
-constexpr int PROJECT_SMEM_DOUBLES_PER_WARP = 32 * PROJ_SEG_PITCH + PROJ_NV * PROJ_MAX_COLS + PROJ_NV * 32;   // tile, running sums, weights
+constexpr int PROJ_SEG_PITCH = 34;  // doubles between consecutive columns of the transposed segment tile
+template <int NV> constexpr int project_smem_doubles_per_warp() {
+    return 32 * PROJ_SEG_PITCH + NV * PROJ_MAX_COLS + (NV > 1 ? 32 * PROJ_NV : 0);   // tile, running sums, weights
+}
 
 struct ProjSegments {
     unsigned short scol[SH_MAX_PROJ];   // slot -> its first column in slot order
@@ -865,92 +872,104 @@ struct ProjSegments {
     unsigned char flush[SH_MAX_PROJ];   // slot -> 1 if the segment is complete after this slot
 };
 
+template <int NV>
 struct ProjectSink {
-    double* tile;        // the warp's [32][PROJ_SEG_PITCH] segment tile
-    double* sums;        // the warp's running sums [PROJ_NV][PROJ_MAX_COLS]
-    const double* wt;    // the tile's weights [PROJ_NV][32]
+    double* tile;        // the warp's [32][PROJ_SEG_PITCH] transposed segment tile
+    double* sums;        // the warp's running sums [NV][PROJ_MAX_COLS]
+    const double* wt;    // NV > 1: the tile's weights [32][PROJ_NV]
     const double* radial;
     const ProjPlan& plan;
     const ProjSegments& seg;
     const RadialPos& pos;
-    int lane, rows, nvec;
+    int lane;
+    double w1;           // NV = 1: this lane's weight
 
     __device__ __forceinline__ void flush(int begin, int len) {
         __syncwarp();
         if (lane < len) {
-            static_for<0, PROJ_NV>([&](auto vc) {
-                constexpr int V = decltype(vc)::value;
-                if (V < nvec) {
-                    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;   // four chains: the FMA latency is not the limit
-                    const double* t = tile + lane;
-                    const double* wv = wt + V * 32;
-                    if (rows == 32) {
+            const double2* t = reinterpret_cast<const double2*>(tile + lane * PROJ_SEG_PITCH);
+            if constexpr (NV == 1) {
+                double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
 #pragma unroll
-                        for (int r = 0; r < 32; r += 4) {
-                            s0 = fma(t[(r + 0) * PROJ_SEG_PITCH], wv[r + 0], s0);
-                            s1 = fma(t[(r + 1) * PROJ_SEG_PITCH], wv[r + 1], s1);
-                            s2 = fma(t[(r + 2) * PROJ_SEG_PITCH], wv[r + 2], s2);
-                            s3 = fma(t[(r + 3) * PROJ_SEG_PITCH], wv[r + 3], s3);
-                        }
-                    } else {
-                        for (int r = 0; r < rows; ++r) s0 = fma(t[r * PROJ_SEG_PITCH], wv[r], s0);
-                    }
-                    sums[V * PROJ_MAX_COLS + begin + lane] += (s0 + s1) + (s2 + s3);
+                for (int r = 0; r < 16; r += 2) {
+                    const double2 a = t[r], b = t[r + 1];
+                    s0 += a.x; s1 += a.y; s2 += b.x; s3 += b.y;
                 }
-            });
+                sums[begin + lane] += (s0 + s1) + (s2 + s3);
+            } else {
+                const double2* wv = reinterpret_cast<const double2*>(wt);   // row r: (w0, w1), (w2, w3)
+                double e[PROJ_NV], o[PROJ_NV];
+                static_for<0, PROJ_NV>([&](auto vc) { e[decltype(vc)::value] = 0.0; o[decltype(vc)::value] = 0.0; });
+#pragma unroll
+                for (int r = 0; r < 16; ++r) {
+                    const double2 a = t[r];   // points 2r, 2r+1
+                    const double2 w01 = wv[4 * r], w23 = wv[4 * r + 1], x01 = wv[4 * r + 2], x23 = wv[4 * r + 3];
+                    e[0] = fma(a.x, w01.x, e[0]); e[1] = fma(a.x, w01.y, e[1]); e[2] = fma(a.x, w23.x, e[2]); e[3] = fma(a.x, w23.y, e[3]);
+                    o[0] = fma(a.y, x01.x, o[0]); o[1] = fma(a.y, x01.y, o[1]); o[2] = fma(a.y, x23.x, o[2]); o[3] = fma(a.y, x23.y, o[3]);
+                }
+                static_for<0, PROJ_NV>([&](auto vc) {
+                    constexpr int V = decltype(vc)::value;
+                    sums[V * PROJ_MAX_COLS + begin + lane] += e[V] + o[V];
+                });
+            }
         }
         __syncwarp();
     }
 
     template <int L> __device__ __forceinline__ void block(const double (&blk)[2 * L + 1]) {
         for (int s = plan.first[L]; s < plan.first[L + 1]; ++s) {
-            const double f = pos.f(radial, plan.nr, plan.chan[s]);
+            double f = pos.f(radial, plan.nr, plan.chan[s]);
+            if constexpr (NV == 1) f *= w1;
             const int c0 = seg.scol[s], b0 = seg.sbeg[s];
-            double* q = tile + lane * PROJ_SEG_PITCH + (c0 - b0);
-            static_for<0, 2 * L + 1>([&](auto mc) { q[decltype(mc)::value] = f * blk[decltype(mc)::value]; });
+            double* q = tile + (c0 - b0) * PROJ_SEG_PITCH + lane;
+            static_for<0, 2 * L + 1>([&](auto mc) { q[decltype(mc)::value * PROJ_SEG_PITCH] = f * blk[decltype(mc)::value]; });
             if (seg.flush[s]) flush(b0, c0 + 2 * L + 1 - b0);
         }
     }
 };
 
-template <int LMAX>
-__global__ void __launch_bounds__(128, 3) sh_project_kernel(const double* __restrict__ xyz, int64_t n, const double* __restrict__ radial,
-                                                             const __grid_constant__ ProjPlan plan, const __grid_constant__ ProjSegments seg,
-                                                             const double* __restrict__ w, int nvec, double* __restrict__ partial) {
+template <int LMAX, int NV>
+__global__ void __launch_bounds__(128, NV == 1 ? 4 : 3) sh_project_kernel(const double* __restrict__ xyz, int64_t n, const double* __restrict__ radial,
+                                                                          const __grid_constant__ ProjPlan plan, const __grid_constant__ ProjSegments seg,
+                                                                          const double* __restrict__ w, int nvec, double* __restrict__ partial) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    double* s_tile = reinterpret_cast<double*>(smem_raw) + (size_t)warp * PROJECT_SMEM_DOUBLES_PER_WARP;
+    double* s_tile = reinterpret_cast<double*>(smem_raw) + (size_t)warp * project_smem_doubles_per_warp<NV>();
     double* s_sums = s_tile + 32 * PROJ_SEG_PITCH;
-    double* s_wt = s_sums + PROJ_NV * PROJ_MAX_COLS;
+    double* s_wt = s_sums + NV * PROJ_MAX_COLS;
     const int ncols = plan.ncols;
-    for (int e = lane; e < PROJ_NV * PROJ_MAX_COLS; e += 32) s_sums[e] = 0.0;
+    for (int e = lane; e < NV * PROJ_MAX_COLS; e += 32) s_sums[e] = 0.0;
     const int64_t ntiles = (n + 31) >> 5;
     const int64_t gw = (int64_t)blockIdx.x * 4 + warp, nw = (int64_t)gridDim.x * 4;
-    // every lane takes part in the warp-level segment sums, so idle lanes of the last tile evaluate a clamped point
-    // (their rows are not summed)
-    auto point_of = [&](int64_t t) { const int64_t i = (t << 5) + lane; return i < n ? i : n - 1; };
-    RawPoint<double> cur, nxt;
-    double wc[PROJ_NV], wn[PROJ_NV];
-    auto load = [&](int64_t t, RawPoint<double>& pt, double (&wv)[PROJ_NV]) {
-        const int64_t i = point_of(t);
-        pt.load(xyz, i);
-        static_for<0, PROJ_NV>([&](auto vc) {
-            constexpr int V = decltype(vc)::value;
-            wv[V] = V < nvec ? __ldg(w + (int64_t)V * n + i) : 0.0;
-        });
+    struct Item { double x, y, z, w[NV]; };
+    auto load = [&](int64_t t, Item& it) {
+        const int64_t i = (t << 5) + lane;
+        if (i < n) {
+            const double* p = xyz + 3 * i;
+            it.x = __ldg(p); it.y = __ldg(p + 1); it.z = __ldg(p + 2);
+            static_for<0, NV>([&](auto vc) {
+                constexpr int V = decltype(vc)::value;
+                it.w[V] = V < nvec ? __ldg(w + (int64_t)V * n + i) : 0.0;
+            });
+        } else {   // idle lane of the ragged last tile: a harmless point with weight 0
+            it.x = 0.0; it.y = 0.0; it.z = 1.0;
+            static_for<0, NV>([&](auto vc) { it.w[decltype(vc)::value] = 0.0; });
+        }
     };
+    Item cur, nxt;
     int64_t t = gw;
-    if (t < ntiles) load(t, cur, wc);
+    if (t < ntiles) load(t, cur);
     for (; t < ntiles; t += nw) {
-        const bool have_next = t + nw < ntiles;
-        if (have_next) load(t + nw, nxt, wn);
-        const int64_t left = n - (t << 5);
-        static_for<0, PROJ_NV>([&](auto vc) { s_wt[decltype(vc)::value * 32 + lane] = wc[decltype(vc)::value]; });
+        if (t + nw < ntiles) load(t + nw, nxt);
+        if constexpr (NV > 1) {
+            // the previous tile's last column sum ended with __syncwarp: the weights may be overwritten
+            reinterpret_cast<double2*>(s_wt)[2 * lane] = make_double2(cur.w[0], cur.w[1]);
+            reinterpret_cast<double2*>(s_wt)[2 * lane + 1] = make_double2(cur.w[2], cur.w[3]);
+        }
         const RadialPos pos(cur.x, cur.y, cur.z, plan);
-        ProjectSink sink{s_tile, s_sums, s_wt, radial, plan, seg, pos, lane, left < 32 ? (int)left : 32, nvec};
-        eval_projector_blocks<LMAX>(cur.unit(SH_COORDS_CARTESIAN), plan, sink);
+        ProjectSink<NV> sink{s_tile, s_sums, s_wt, radial, plan, seg, pos, lane, cur.w[0]};
+        eval_projector_blocks<LMAX>(normalize(cur.x, cur.y, cur.z), plan, sink);
         cur = nxt;
-        static_for<0, PROJ_NV>([&](auto vc) { wc[decltype(vc)::value] = wn[decltype(vc)::value]; });
     }
     __syncwarp();
     for (int v = 0; v < nvec; ++v)
@@ -1338,7 +1357,7 @@ int check_projector_args(const double* xyz, int64_t n, int nproj, const int* pro
     return SH_OK;
 }
 
-constexpr int PROJ_CTAS_PER_SM = 3;   // grid of sh_project_kernel: the machine filled once (what the workspace is sized for)
+constexpr int PROJ_CTAS_PER_SM = 4;   // grid cap of sh_project_kernel: the machine filled once (what the workspace is sized for)
 
 template <int LMAX>
 int launch_proj_aos(const double* xyz, int64_t n, const double* radial, const ProjPlan& plan, double* out, cudaStream_t st) {
@@ -1422,16 +1441,21 @@ int launch_project(const double* xyz, int64_t n, const double* radial, const Pro
                    double* partial, double* coeff, int coeff_stride, cudaStream_t st) {
     const int64_t ntiles = (n + 31) / 32;
     int64_t blocks = (ntiles + 3) / 4;
-    const int64_t cap = (int64_t)sm_count() * PROJ_CTAS_PER_SM;
+    const int64_t cap = (int64_t)sm_count() * (nvec == 1 ? PROJ_CTAS_PER_SM : PROJ_CTAS_PER_SM - 1);   // resident CTAs per SM (__launch_bounds__)
     if (blocks > cap) blocks = cap;
-    constexpr size_t smem = (size_t)4 * PROJECT_SMEM_DOUBLES_PER_WARP * sizeof(double);   // 53 KB: above the 48 KB default
-    static bool opted_in = false;
-    if (!opted_in) {
-        cudaError_t e = cudaFuncSetAttribute(sh_project_kernel<LMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return cuda_fail(e);
-        opted_in = true;
+    if (nvec == 1) {
+        constexpr size_t smem = (size_t)4 * project_smem_doubles_per_warp<1>() * sizeof(double);   // 38 KB
+        sh_project_kernel<LMAX, 1><<<(unsigned)blocks, 128, smem, st>>>(xyz, n, radial, plan, seg, w, nvec, partial);
+    } else {
+        constexpr size_t smem = (size_t)4 * project_smem_doubles_per_warp<PROJ_NV>() * sizeof(double);   // 54 KB: above the 48 KB default
+        static bool opted_in = false;
+        if (!opted_in) {
+            cudaError_t e = cudaFuncSetAttribute(sh_project_kernel<LMAX, PROJ_NV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return cuda_fail(e);
+            opted_in = true;
+        }
+        sh_project_kernel<LMAX, PROJ_NV><<<(unsigned)blocks, 128, smem, st>>>(xyz, n, radial, plan, seg, w, nvec, partial);
     }
-    sh_project_kernel<LMAX><<<(unsigned)blocks, 128, smem, st>>>(xyz, n, radial, plan, seg, w, nvec, partial);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
