@@ -167,10 +167,13 @@ def run_reference(args):
     print(json.dumps(line))
 
 
-def extra_configs(sh, dev):
-    """The other BASELINE.json configs, timed with CUDA events outside the headline's timed region (context, not `value`)."""
+def extra_configs(sh, dev, only=None):
+    """The other BASELINE.json configs, timed with CUDA events outside the headline's timed region (context, not `value`).
+    `only`: run just the cases whose name contains this substring (what the ncu captures under profiles/ use)."""
     import torch
     from paper_2510_05282_b200 import inputs
+
+    want = lambda name: only is None or only in name
 
     def timed(fn, reps):
         for _ in range(3):
@@ -193,6 +196,8 @@ def extra_configs(sh, dev):
     ang = np.ascontiguousarray(np.stack([np.arccos(np.clip(unit[:, 2], -1, 1)), np.arctan2(unit[:, 1], unit[:, 0])], axis=1))
     out = torch.empty((K, len(grid)), dtype=torch.float64, device=dev)
     for coords, arr in (("cartesian", grid), ("normalized", unit), ("angular", ang)):
+        if not want(f"config3 real l9 SoA front end {coords}"):
+            continue
         x = torch.from_numpy(arr).to(dev)
         ms = timed(lambda: sh.sh_real(x, LMAX, out=out, layout="soa", coords=coords), 20)
         res[f"config3 real l9 SoA front end {coords}"] = {"ms": ms, "write_GBps": len(grid) * K * 8 / ms / 1e6, "G_values_per_s": len(grid) * K / ms / 1e6}
@@ -210,12 +215,16 @@ def extra_configs(sh, dev):
         ("ext complex l32 N=2^20", "complex_ext", inputs.config5_ball(n=1 << 20), 32, ["soa"], 3),
     ]
     for name, kind, pts, lmax, layouts, reps in cases:
+        if not any(want(f"{name} {layout}") for layout in layouts):
+            continue
         x = torch.from_numpy(pts).to(dev)
         n = len(pts)
         per_point = sh.count(kind, lmax)
         esize = 4 if kind == "real_f32" else 8
         values = {"real": 1, "real_f32": 1, "real_ext": 1, "complex": 2, "complex_ext": 2, "spinor": 2}[kind]  # scalars per "value" (a complex number is one value)
         for layout in layouts:
+            if not want(f"{name} {layout}"):
+                continue
             out = torch.empty(sh.out_shape(kind, n, lmax, layout), dtype=x.dtype, device=dev)
             fn = getattr(sh, "sh_" + kind)
             ms = timed(lambda: fn(x, lmax, out=out, layout=layout), reps)
@@ -226,7 +235,79 @@ def extra_configs(sh, dev):
             del out
         del x
         torch.cuda.empty_cache()
+    res.update(projector_cases(sh, dev, timed, want))
     return res
+
+
+# FP64 pipe peak for the ALU-bound fused projection: 64 FP64 lanes per SM per clock (B300_MICROARCH.md
+# unit counts; confirmed here by a DFMA microbenchmark: 36.7 TFLOP/s = 148 x 64 x 2 x 1.94 GHz), one DADD/DMUL/DFMA = one
+# lane-slot.  Peak = 148 SMs x 64 lanes x clock; the clock is the nvidia-smi maximum (1965 MHz), so power-capped runs read low.
+FP64_LANES_PER_SM = 64
+N_SMS = 148
+SM_MAX_GHZ = 1.965
+
+
+def projector_cases(sh, dev, timed, want):
+    """Fused projector consumer: sh_projectors (stores only the requested columns) and sh_project
+    (contraction with weight vectors; writes nothing per point, FP64-pipe bound)."""
+    import torch
+    from paper_2510_05282_b200 import inputs
+
+    res = {}
+    peak_ginstr = N_SMS * FP64_LANES_PER_SM * SM_MAX_GHZ  # G FP64 lane-instructions/s
+    work = [
+        # name, points, (lmax, per_l, cutoff, dr), volume element
+        ("config2 grid l3 x2 channels (32 cols)", inputs.config2_projector_grid(), (3, 2, 3.0, 0.01), 1e-3),
+        ("128^3 grid l9 x1 channel (100 cols)", inputs.config3_full_grid(), (9, 1, 6.0, 0.02), (12.0 / 128) ** 3),
+    ]
+    for name, pts, (lmax, per_l, cutoff, dr), dv in work:
+        if not any(want(f"{k} {name}") for k in ("projectors soa", "projectors aos", "project nvec=1", "project nvec=4")):
+            continue
+        n = len(pts)
+        proj_l, tab, dr = inputs.projector_channels(lmax=lmax, per_l=per_l, cutoff=cutoff, dr=dr)
+        ncols = sh.projector_count(proj_l)
+        x = torch.from_numpy(pts).to(dev)
+        t = torch.from_numpy(tab).to(dev)
+        reps = 50 if n < (1 << 20) else 20
+        for layout in ("soa", "aos"):
+            if not want(f"projectors {layout} {name}"):
+                continue
+            out = torch.empty((ncols, n) if layout == "soa" else (n, ncols), dtype=torch.float64, device=dev)
+            ms = timed(lambda: sh.sh_projectors(x, proj_l, t, dr, out=out, layout=layout), reps)
+            res[f"projectors {layout} {name}"] = {"ms": ms, "write_GBps": n * ncols * 8 / ms / 1e6, "G_values_per_s": n * ncols / ms / 1e6}
+            if layout == "aos" and os.environ.get("SHB200_BENCH_SWEEP"):
+                for mode in (1, 2, 3):
+                    sh.set_tuning("proj_aos_mode", mode)
+                    res[f"projectors {layout} {name}"][f"ms_mode{mode}"] = timed(lambda: sh.sh_projectors(x, proj_l, t, dr, out=out, layout=layout), reps)
+                sh.set_tuning("proj_aos_mode", 0)
+            del out
+        for nvec in (1, 4):
+            if not want(f"project nvec={nvec} {name}"):
+                continue
+            w = torch.from_numpy(inputs.wave_weights(n, nvec, seed=8, volume_element=dv)).to(dev)
+            coeff = torch.empty((nvec, ncols), dtype=torch.float64, device=dev)
+            ws = torch.empty(max(sh.project_workspace_bytes(ncols, nvec), 8), dtype=torch.uint8, device=dev)
+            ms = timed(lambda: sh.sh_project(x, proj_l, t, dr, w, coeff=coeff, workspace=ws), reps)
+            # algorithmic FP64 work per point: DESIGN.md section 6 "fused projection" (instruction counts of the evaluated blocks
+            # + ncols (radial scale) + nvec x ncols (contraction)); reported against the FP64 pipe
+            fp64_per_point = PROJECT_FP64_PER_POINT.get(lmax, 0) + ncols + nvec * ncols
+            res[f"project nvec={nvec} {name}"] = {
+                "ms": ms, "G_points_per_s": n / ms / 1e6, "G_values_per_s": n * ncols * nvec / ms / 1e6,
+                "read_GBps": n * (24 + 8 * nvec) / ms / 1e6,
+                "roofline": {"bound": "alu", "unit": "G FP64 lane-instr/s", "achieved": n * fp64_per_point / ms / 1e6,
+                             "peak": peak_ginstr, "frac": n * fp64_per_point / ms / 1e6 / peak_ginstr,
+                             "fp64_instr_per_point": fp64_per_point},
+            }
+            del w, coeff, ws
+        del x, t
+        torch.cuda.empty_cache()
+    return res
+
+
+# FP64 instructions (DADD + DMUL + DFMA in SASS, one lane-slot each) per point of steps a2-a5 for all blocks l <= lmax, as
+# compiled for the store kernels (cuobjdump: 94 at lmax = 3, 566 at lmax = 9), plus the radial position (sqrt, ~12) and the
+# table interpolation (3 per channel: 8 / 10 channels); DESIGN.md section 6.  Keys = lmax.
+PROJECT_FP64_PER_POINT = {3: 94 + 12 + 24, 9: 566 + 12 + 30}
 
 
 def run_ours(args):
@@ -352,7 +433,7 @@ def run_ours(args):
         if world == 1 and not args.no_extras:
             del out_soa, out_aos, xs
             torch.cuda.empty_cache()
-            line["other_configs"] = extra_configs(sh, dev)
+            line["other_configs"] = extra_configs(sh, dev, args.only)
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(pts)
         print(json.dumps(line))
@@ -368,6 +449,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the untimed-by-`value` runs of the other configs")
+    ap.add_argument("--only", default=None, help="run only the other-config cases whose name contains this substring")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -16,6 +16,7 @@ from .binding import (  # noqa: F401
     out_shape,
     project_workspace_bytes,
     projector_count,
+    set_tuning,
     lmax_ext,
     sh_complex,
     sh_complex_ext,

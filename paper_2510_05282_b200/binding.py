@@ -110,6 +110,19 @@ def index_spinor(l: int, twoj: int, twomj: int) -> int:
     return load().sh_index_spinor(l, twoj, twomj)
 
 
+TUNE = {"soa_tiles_per_cta": 0, "aos_tiles_per_warp": 1, "prefetch_window_points": 2, "proj_aos_mode": 3}
+
+
+def set_tuning(knob, value: int) -> None:
+    """sh_set_tuning: override a launch heuristic (include/shb200.h SH_TUNE_*); value 0 restores the default."""
+    lib = load()
+    lib.sh_set_tuning.argtypes = [ctypes.c_int, ctypes.c_int]
+    lib.sh_set_tuning.restype = ctypes.c_int
+    rc = lib.sh_set_tuning(TUNE[knob] if isinstance(knob, str) else int(knob), int(value))
+    if rc != 0:
+        raise ShError(rc, "sh_set_tuning")
+
+
 def kernel_launch_count() -> int:
     return int(load().sh_kernel_launch_count())
 

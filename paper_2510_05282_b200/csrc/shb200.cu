@@ -744,6 +744,17 @@ struct RadialPos {
     }
 };
 
+// Radial values of EVERY channel slot at this lane's point, computed up front and parked in shared memory as
+// fs[slot*32 + lane] (times `scale`).  The table loads of different slots are independent, so their latencies overlap;
+// loaded one l-block at a time instead, a warp pays one dependent L2 round trip per channel (the staging tiles leave
+// little L1), which is what bounds the low-occupancy staging kernels (AoS sh_projectors 0.41 -> see DESIGN.md section 6).
+__device__ __forceinline__ void stage_radial(const RadialPos& pos, const double* __restrict__ radial, const ProjPlan& plan, double* fs, int lane,
+                                             double scale) {
+    const int nslots = plan.first[shgen::LMAX_CAP + 1];
+#pragma unroll 4
+    for (int s = 0; s < nslots; ++s) fs[s * 32 + lane] = pos.f(radial, plan.nr, plan.chan[s]) * scale;
+}
+
 // the real harmonics of block l in ascending m (a3-a5), handed to the sink one block at a time
 template <int LMAX, class Sink>
 __device__ __forceinline__ void eval_projector_blocks(const UnitVec& u, const ProjPlan& plan, Sink& sink) {
@@ -798,16 +809,22 @@ __global__ void __launch_bounds__(256) sh_proj_soa_kernel(const double* __restri
 }
 
 // sh_projectors, AoS: one warp = one 32-point tile.  Each lane stages its point's row in the warp's shared-memory tile
-// (pitch odd: conflict-free 8-byte stores); the tile is one contiguous span of `out`, copied out by the warp with coalesced
-// streaming stores.
+// with 8-byte stores at runtime column offsets; the tile is one contiguous span of `out`.  Copy-out, by `mode`:
+//   PROJ_AOS_TILEBULK (`out` 16-byte aligned, ncols not a multiple of 8): rows staged densely (pitch = ncols; the 8-byte
+//       staging stores conflict gcd(ncols, 16)-way, i.e. not at all for odd ncols), one TMA bulk copy
+//       (cp.async.bulk.global.shared::cta) of the whole tile by lane 0; one warp per CTA (see TILEBULK_WARPS);
+//   PROJ_AOS_ROWBULK (ncols a multiple of 8, `out` 16-byte aligned): pitch = ncols + 2 (rows stay 16-byte aligned, staging
+//       stores conflict 2-way), one bulk copy per row by its lane (32 copies issued one after the other);
+//   PROJ_AOS_PLAIN: pitch odd, the warp copies the tile out with coalesced streaming stores (any alignment, any width).
+// A ragged last tile is always copied out by the warp.
+constexpr int PROJ_AOS_PLAIN = 0, PROJ_AOS_ROWBULK = 1, PROJ_AOS_TILEBULK = 2;
 struct ProjRowSink {
     double* row;
-    const double* radial;
+    const double* fs;   // this lane's radial values: fs[slot*32]
     const ProjPlan& plan;
-    const RadialPos& pos;
     template <int L> __device__ __forceinline__ void block(const double (&blk)[2 * L + 1]) {
         for (int s = plan.first[L]; s < plan.first[L + 1]; ++s) {
-            const double f = pos.f(radial, plan.nr, plan.chan[s]);
+            const double f = fs[s * 32];
             double* q = row + plan.col[s];
             static_for<0, 2 * L + 1>([&](auto mc) { q[decltype(mc)::value] = f * blk[decltype(mc)::value]; });
         }
@@ -816,12 +833,15 @@ struct ProjRowSink {
 
 template <int LMAX>
 __global__ void __launch_bounds__(128) sh_proj_aos_kernel(const double* __restrict__ xyz, int64_t n, const double* __restrict__ radial,
-                                                           const __grid_constant__ ProjPlan plan, double* __restrict__ out, InputPrefetch pf) {
+                                                           const __grid_constant__ ProjPlan plan, double* __restrict__ out, int pitch, int mode,
+                                                           InputPrefetch pf) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, warps = blockDim.x >> 5;
     prefetch_input_window(xyz, n * 24, (int64_t)warps * 32 * 24, pf);
-    const int ncols = plan.ncols, pitch = ncols | 1;
-    double* tile = reinterpret_cast<double*>(smem_raw) + (size_t)warp * 32 * pitch;
+    const int ncols = plan.ncols;
+    const int nslots = plan.first[shgen::LMAX_CAP + 1];
+    double* tile = reinterpret_cast<double*>(smem_raw) + (size_t)warp * 32 * (pitch + nslots);
+    double* fs = tile + 32 * pitch;   // radial values [slot][lane]
     const int64_t base = ((int64_t)blockIdx.x * warps + warp) << 5;
     if (base >= n) return;
     const int64_t i = base + lane;
@@ -830,11 +850,27 @@ __global__ void __launch_bounds__(128) sh_proj_aos_kernel(const double* __restri
         RawPoint<double> pt;
         pt.load(xyz, i);
         const RadialPos pos(pt.x, pt.y, pt.z, plan);
-        ProjRowSink sink{tile + lane * pitch, radial, plan, pos};
+        stage_radial(pos, radial, plan, fs, lane, 1.0);
+        ProjRowSink sink{tile + lane * pitch, fs + lane, plan};
         eval_projector_blocks<LMAX>(pt.unit(SH_COORDS_CARTESIAN), plan, sink);
     }
-    __syncwarp();
     double* g = out + base * ncols;
+    if (mode != PROJ_AOS_PLAIN && rows == 32) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // every lane: its staging stores -> async proxy
+        if (mode == PROJ_AOS_TILEBULK) {
+            __syncwarp();
+            if (lane == 0)
+                asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(g), "r"(smem_u32(tile)), "r"(32 * ncols * 8) : "memory");
+        } else {
+            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(g + (int64_t)lane * ncols),
+                         "r"(smem_u32(tile + lane * pitch)), "r"(ncols * 8)
+                         : "memory");
+        }
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory is released when the CTA exits
+        return;
+    }
+    __syncwarp();
     const int total = rows * ncols;
     int r = 0, c = lane;
     while (c >= ncols) { c -= ncols; ++r; }
@@ -877,12 +913,10 @@ struct ProjectSink {
     double* tile;        // the warp's [32][PROJ_SEG_PITCH] transposed segment tile
     double* sums;        // the warp's running sums [NV][PROJ_MAX_COLS]
     const double* wt;    // NV > 1: the tile's weights [32][PROJ_NV]
-    const double* radial;
+    const double* fs;    // this lane's radial values fs[slot*32] (NV = 1: times the lane's weight)
     const ProjPlan& plan;
     const ProjSegments& seg;
-    const RadialPos& pos;
     int lane;
-    double w1;           // NV = 1: this lane's weight
 
     __device__ __forceinline__ void flush(int begin, int len) {
         __syncwarp();
@@ -918,8 +952,7 @@ struct ProjectSink {
 
     template <int L> __device__ __forceinline__ void block(const double (&blk)[2 * L + 1]) {
         for (int s = plan.first[L]; s < plan.first[L + 1]; ++s) {
-            double f = pos.f(radial, plan.nr, plan.chan[s]);
-            if constexpr (NV == 1) f *= w1;
+            const double f = fs[s * 32];
             const int c0 = seg.scol[s], b0 = seg.sbeg[s];
             double* q = tile + (c0 - b0) * PROJ_SEG_PITCH + lane;
             static_for<0, 2 * L + 1>([&](auto mc) { q[decltype(mc)::value * PROJ_SEG_PITCH] = f * blk[decltype(mc)::value]; });
@@ -934,9 +967,11 @@ __global__ void __launch_bounds__(128, NV == 1 ? 4 : 3) sh_project_kernel(const 
                                                                           const double* __restrict__ w, int nvec, double* __restrict__ partial) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    double* s_tile = reinterpret_cast<double*>(smem_raw) + (size_t)warp * project_smem_doubles_per_warp<NV>();
+    const int nslots = plan.first[shgen::LMAX_CAP + 1];
+    double* s_tile = reinterpret_cast<double*>(smem_raw) + (size_t)warp * (project_smem_doubles_per_warp<NV>() + 32 * nslots);
     double* s_sums = s_tile + 32 * PROJ_SEG_PITCH;
     double* s_wt = s_sums + NV * PROJ_MAX_COLS;
+    double* s_fs = s_tile + project_smem_doubles_per_warp<NV>();   // radial values [slot][lane]
     const int ncols = plan.ncols;
     for (int e = lane; e < NV * PROJ_MAX_COLS; e += 32) s_sums[e] = 0.0;
     const int64_t ntiles = (n + 31) >> 5;
@@ -967,7 +1002,8 @@ __global__ void __launch_bounds__(128, NV == 1 ? 4 : 3) sh_project_kernel(const 
             reinterpret_cast<double2*>(s_wt)[2 * lane + 1] = make_double2(cur.w[2], cur.w[3]);
         }
         const RadialPos pos(cur.x, cur.y, cur.z, plan);
-        ProjectSink<NV> sink{s_tile, s_sums, s_wt, radial, plan, seg, pos, lane, cur.w[0]};
+        stage_radial(pos, radial, plan, s_fs, lane, NV == 1 ? cur.w[0] : 1.0);   // only this lane reads its column back
+        ProjectSink<NV> sink{s_tile, s_sums, s_wt, s_fs + lane, plan, seg, lane};
         eval_projector_blocks<LMAX>(normalize(cur.x, cur.y, cur.z), plan, sink);
         cur = nxt;
     }
@@ -1362,8 +1398,23 @@ constexpr int PROJ_CTAS_PER_SM = 4;   // grid cap of sh_project_kernel: the mach
 template <int LMAX>
 int launch_proj_aos(const double* xyz, int64_t n, const double* radial, const ProjPlan& plan, double* out, cudaStream_t st) {
     auto kern = sh_proj_aos_kernel<LMAX>;
-    const size_t per_warp = (size_t)32 * (plan.ncols | 1) * sizeof(double);
-    int warps = 4;
+    const int ncols = plan.ncols;
+    // store mode (see the kernel): bulk copies need a 16-byte aligned `out` and a tile that leaves room for >= 4 CTAs per SM
+    int mode = PROJ_AOS_PLAIN, pitch = ncols | 1, warps = 4;
+    if (aligned(out, 16) && (size_t)32 * (ncols + 2 + plan.first[shgen::LMAX_CAP + 1]) * sizeof(double) <= (size_t)55 * 1024) {
+        // dense rows conflict gcd(ncols, 16)-way on the 8-byte staging stores (16 lanes per wavefront, rows ncols words apart)
+        int g = 16;
+        while (ncols % g) g >>= 1;
+        mode = g <= 4 ? PROJ_AOS_TILEBULK : PROJ_AOS_ROWBULK;
+        const int force = tuned(SH_TUNE_PROJ_AOS_MODE, 0);
+        if (force == 1) mode = PROJ_AOS_PLAIN;
+        else if (force == 2 && ncols % 2 == 0) mode = PROJ_AOS_ROWBULK;
+        else if (force == 3) mode = PROJ_AOS_TILEBULK;
+        if (mode == PROJ_AOS_TILEBULK) pitch = ncols;
+        else if (mode == PROJ_AOS_ROWBULK) pitch = (ncols / 2) & 1 ? ncols : ncols + 2;
+        if (mode != PROJ_AOS_PLAIN) warps = TILEBULK_WARPS;   // fence.proxy.async is CTA-scoped: one warp per CTA keeps the warps' copies independent
+    }
+    const size_t per_warp = (size_t)32 * (pitch + plan.first[shgen::LMAX_CAP + 1]) * sizeof(double);   // row tile + radial values
     while (warps > 1 && warps * per_warp > (size_t)56 * 1024) warps >>= 1;   // four CTAs per SM while the row width allows it
     const size_t smem = warps * per_warp;
     if (smem > (size_t)227 * 1024) return SH_ERR_PROJECTOR;
@@ -1376,7 +1427,7 @@ int launch_proj_aos(const double* xyz, int64_t n, const double* radial, const Pr
     const int64_t ntiles = (n + 31) / 32;
     const int64_t blocks = (ntiles + warps - 1) / warps;
     if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
-    kern<<<(unsigned)blocks, warps * 32, smem, st>>>(xyz, n, radial, plan, out, prefetch_plan(n, (int64_t)warps * 32));
+    kern<<<(unsigned)blocks, warps * 32, smem, st>>>(xyz, n, radial, plan, out, pitch, mode, prefetch_plan(n, (int64_t)warps * 32));
     g_launches.fetch_add(1, std::memory_order_relaxed);
     cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? SH_OK : cuda_fail(e);
@@ -1443,16 +1494,24 @@ int launch_project(const double* xyz, int64_t n, const double* radial, const Pro
     int64_t blocks = (ntiles + 3) / 4;
     const int64_t cap = (int64_t)sm_count() * (nvec == 1 ? PROJ_CTAS_PER_SM : PROJ_CTAS_PER_SM - 1);   // resident CTAs per SM (__launch_bounds__)
     if (blocks > cap) blocks = cap;
+    // per warp: segment tile, running sums, (weights,) and the radial values of every slot: 38 / 54 KB + 1 KB per slot per CTA
+    const size_t slots_bytes = (size_t)4 * 32 * plan.first[shgen::LMAX_CAP + 1] * sizeof(double);
+    constexpr size_t smem_max = (size_t)4 * (project_smem_doubles_per_warp<PROJ_NV>() + 32 * SH_MAX_PROJ) * sizeof(double);   // 86 KB
+    static bool opted_in[2] = {false, false};
     if (nvec == 1) {
-        constexpr size_t smem = (size_t)4 * project_smem_doubles_per_warp<1>() * sizeof(double);   // 38 KB
+        const size_t smem = (size_t)4 * project_smem_doubles_per_warp<1>() * sizeof(double) + slots_bytes;
+        if (!opted_in[0]) {
+            cudaError_t e = cudaFuncSetAttribute(sh_project_kernel<LMAX, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
+            if (e != cudaSuccess) return cuda_fail(e);
+            opted_in[0] = true;
+        }
         sh_project_kernel<LMAX, 1><<<(unsigned)blocks, 128, smem, st>>>(xyz, n, radial, plan, seg, w, nvec, partial);
     } else {
-        constexpr size_t smem = (size_t)4 * project_smem_doubles_per_warp<PROJ_NV>() * sizeof(double);   // 54 KB: above the 48 KB default
-        static bool opted_in = false;
-        if (!opted_in) {
-            cudaError_t e = cudaFuncSetAttribute(sh_project_kernel<LMAX, PROJ_NV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        const size_t smem = (size_t)4 * project_smem_doubles_per_warp<PROJ_NV>() * sizeof(double) + slots_bytes;
+        if (!opted_in[1]) {
+            cudaError_t e = cudaFuncSetAttribute(sh_project_kernel<LMAX, PROJ_NV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
             if (e != cudaSuccess) return cuda_fail(e);
-            opted_in = true;
+            opted_in[1] = true;
         }
         sh_project_kernel<LMAX, PROJ_NV><<<(unsigned)blocks, 128, smem, st>>>(xyz, n, radial, plan, seg, w, nvec, partial);
     }

@@ -113,6 +113,29 @@ def test_every_lmax_unsorted_channels_and_ragged_sizes(sh, oracle_mod, lmax):
         check_project(gpu_project(sh, pts, proj_l, tab, dr, w), coeff, abs_sum)
 
 
+@pytest.mark.parametrize("proj_l", [[2], [0, 1, 3], [1, 1], [0, 2, 1, 3], [9, 9, 9, 4, 0], [9] * 11, [9] * 12])
+def test_aos_store_modes(sh, oracle_mod, proj_l):
+    """AoS copy-out modes of sh_projectors: odd ncols (one bulk copy per tile), even ncols with ncols/2 odd or even (one
+    bulk copy per row, padded pitch), rows too wide for the bulk tile (12 x 19 = 228 columns), a misaligned `out` (warp copy);
+    full tiles, a ragged tail and fewer points than one tile."""
+    rng = np.random.default_rng(len(proj_l) * 31 + proj_l[0])
+    nr, dr = 33, 0.1
+    tab = rng.standard_normal((len(proj_l), nr))
+    tab[:, -1] = 0.0
+    for n in (7, 64, 1000 + 13):
+        g = rng.standard_normal((n, 3))
+        pts = g / np.linalg.norm(g, axis=1)[:, None] * rng.uniform(0.0, 3.5, n)[:, None]
+        want = oracle_mod.projectors(pts, proj_l, tab, dr)
+        for mis in (0, 1, 2):
+            for mode in (0, 1, 2, 3):   # automatic, then each copy-out forced (where it applies)
+                sh.set_tuning("proj_aos_mode", mode)
+                try:
+                    got = gpu_projectors(sh, pts, proj_l, tab, dr, "aos", misalign=mis)
+                finally:
+                    sh.set_tuning("proj_aos_mode", 0)
+                assert np.abs(got - want).max() <= TOL * max(1.0, np.abs(tab).max()), (n, mis, mode)
+
+
 def test_many_channels_wide_rows(sh, oracle_mod):
     """32 channels of l = 9: 608 columns -- the AoS tile is 156 KB (one warp per CTA) and the projection runs as five
     launches of at most 128 columns."""
