@@ -187,6 +187,28 @@ def extra_configs(sh, dev, only=None):
         torch.cuda.synchronize()
         return a.elapsed_time(b) / reps
 
+    def timed_graph(fn, reps):
+        """The same call captured `reps` times in one CUDA graph (the library allocates nothing and is asynchronous on the
+        stream it is given, so it can be captured): per-call time without the Python/ctypes launch overhead."""
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            fn()
+        torch.cuda.current_stream().wait_stream(side)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            for _ in range(reps):
+                fn()
+        g.replay()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        g.replay()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+
     res = {}
     # the paper's three front ends (P:69, Table I P:144-151) on the headline workload, SoA
     grid = inputs.config3_full_grid()
@@ -232,10 +254,12 @@ def extra_configs(sh, dev, only=None):
                 "ms": ms, "write_GBps": n * per_point * esize / ms / 1e6,
                 "G_values_per_s": n * per_point / values / ms / 1e6,
             }
+            if n < (1 << 18):   # launch-bound sizes: also as CUDA-graph replays
+                res[f"{name} {layout}"]["ms_in_cuda_graph"] = timed_graph(lambda: fn(x, lmax, out=out, layout=layout), 100)
             del out
         del x
         torch.cuda.empty_cache()
-    res.update(projector_cases(sh, dev, timed, want))
+    res.update(projector_cases(sh, dev, timed, timed_graph, want))
     return res
 
 
@@ -247,7 +271,7 @@ N_SMS = 148
 SM_MAX_GHZ = 1.965
 
 
-def projector_cases(sh, dev, timed, want):
+def projector_cases(sh, dev, timed, timed_graph, want):
     """Fused projector consumer: sh_projectors (stores only the requested columns) and sh_project
     (contraction with weight vectors; writes nothing per point, FP64-pipe bound)."""
     import torch
@@ -275,6 +299,8 @@ def projector_cases(sh, dev, timed, want):
             out = torch.empty((ncols, n) if layout == "soa" else (n, ncols), dtype=torch.float64, device=dev)
             ms = timed(lambda: sh.sh_projectors(x, proj_l, t, dr, out=out, layout=layout), reps)
             res[f"projectors {layout} {name}"] = {"ms": ms, "write_GBps": n * ncols * 8 / ms / 1e6, "G_values_per_s": n * ncols / ms / 1e6}
+            if n < (1 << 18):
+                res[f"projectors {layout} {name}"]["ms_in_cuda_graph"] = timed_graph(lambda: sh.sh_projectors(x, proj_l, t, dr, out=out, layout=layout), 100)
             if layout == "aos" and os.environ.get("SHB200_BENCH_SWEEP"):
                 for mode in (1, 2, 3):
                     sh.set_tuning("proj_aos_mode", mode)
@@ -288,6 +314,8 @@ def projector_cases(sh, dev, timed, want):
             coeff = torch.empty((nvec, ncols), dtype=torch.float64, device=dev)
             ws = torch.empty(max(sh.project_workspace_bytes(ncols, nvec), 8), dtype=torch.uint8, device=dev)
             ms = timed(lambda: sh.sh_project(x, proj_l, t, dr, w, coeff=coeff, workspace=ws), reps)
+            if n < (1 << 18):   # launch-bound: the roofline below uses the CUDA-graph time
+                ms_py, ms = ms, timed_graph(lambda: sh.sh_project(x, proj_l, t, dr, w, coeff=coeff, workspace=ws), 100)
             # algorithmic FP64 work per point: DESIGN.md section 6 "fused projection" (instruction counts of the evaluated blocks
             # + ncols (radial scale) + nvec x ncols (contraction)); reported against the FP64 pipe
             fp64_per_point = PROJECT_FP64_PER_POINT.get(lmax, 0) + ncols + nvec * ncols
@@ -298,6 +326,8 @@ def projector_cases(sh, dev, timed, want):
                              "peak": peak_ginstr, "frac": n * fp64_per_point / ms / 1e6 / peak_ginstr,
                              "fp64_instr_per_point": fp64_per_point},
             }
+            if n < (1 << 18):
+                res[f"project nvec={nvec} {name}"].update({"ms": ms_py, "ms_in_cuda_graph": ms})
             del w, coeff, ws
         del x, t
         torch.cuda.empty_cache()

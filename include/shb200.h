@@ -124,7 +124,7 @@ int sh_lmax_ext(void);
  * sh_projectors: out[i*ncols + col] (SH_LAYOUT_AOS) or out[col*n + i] (SH_LAYOUT_SOA) = beta_col(xyz_i); only the
  *   requested channels are evaluated and written (8 ncols bytes per point instead of 800).
  * sh_project: coeff[v*ncols + col] = sum_i w[v*n + i] beta_col(xyz_i), v < nvec: the projection <beta|psi> with
- *   w = psi dV; NOTHING per point is written.  The sum is taken in a fixed order (per-warp partial sums in `workspace`,
+ *   w = psi dV; NOTHING per point is written.  The sum is taken in a fixed order (per-CTA partial sums in `workspace`,
  *   then one ordered pass), so results are reproducible run to run on one device; they differ from the sum in point
  *   order by rounding only (<= 1e-12 sum_i |w_i beta_i| is the tested bound).  `workspace` must hold at least
  *   sh_project_workspace_bytes(ncols, nvec) bytes, 8-byte aligned; its contents are scratch. */

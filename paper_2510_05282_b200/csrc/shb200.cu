@@ -892,9 +892,9 @@ __global__ void __launch_bounds__(128) sh_proj_aos_kernel(const double* __restri
 //   NV = 1: the weight is folded into the radial value (beta w is staged), the column sum is 32 additions;
 //   NV = 4: up to four weight vectors; the tile's weights sit in shared memory as [point][4] and are read as broadcasts.
 // Idle lanes of a ragged last tile evaluate the point (0, 0, 1) with weight 0, so every column sum runs over 32 rows.
-// Running sums are kept in the order of production ("slot order"); every warp writes them to `partial`
-// [warp][nvec][ncols] at the end, and sh_project_reduce_kernel adds the warps in a fixed order and scatters to the
-// caller's column order.
+// Running sums are kept in the order of production ("slot order"); at the end a CTA adds its four warps in a fixed order
+// and writes one row of `partial` [cta][nvec][ncols]; sh_project_reduce_kernel adds the rows in a fixed order and
+// scatters to the caller's column order.
 constexpr int PROJ_NV = 4;          // weight vectors contracted per launch
 constexpr int PROJ_MAX_COLS = 128;  // columns per launch (whole channels); wider channel lists run as several launches
 constexpr int PROJ_SEG_PITCH = 34;  // doubles between consecutive columns of the transposed segment tile
@@ -1007,36 +1007,42 @@ __global__ void __launch_bounds__(128, NV == 1 ? 4 : 3) sh_project_kernel(const 
         eval_projector_blocks<LMAX>(normalize(cur.x, cur.y, cur.z), plan, sink);
         cur = nxt;
     }
-    __syncwarp();
-    for (int v = 0; v < nvec; ++v)
-        for (int c = lane; c < ncols; c += 32) partial[(gw * nvec + v) * ncols + c] = s_sums[v * PROJ_MAX_COLS + c];
+    // the CTA's four warps are added in a fixed order: one row of `partial` per CTA
+    __syncthreads();
+    const size_t wstride = project_smem_doubles_per_warp<NV>() + 32 * nslots;
+    const double* s0 = reinterpret_cast<const double*>(smem_raw) + 32 * PROJ_SEG_PITCH;
+    for (int e = threadIdx.x; e < nvec * ncols; e += 128) {
+        const int v = e / ncols, c = e - v * ncols;
+        const double* q = s0 + v * PROJ_MAX_COLS + c;
+        partial[(int64_t)blockIdx.x * nvec * ncols + e] = ((q[0] + q[wstride]) + q[2 * wstride]) + q[3 * wstride];
+    }
 }
 
-// coeff[v*coeff_stride + user column] = sum over warps of partial[warp][v][slot-order column], the warps added in a fixed
-// order (reproducible): 32 lanes = 32 consecutive (v, column) elements; the block's 16 warps each add every 16th warp of
-// `partial` (coalesced, four loads in flight), then the 16 sums are added in order.
-__global__ void __launch_bounds__(512) sh_project_reduce_kernel(const double* __restrict__ partial, int nwarps, int nvec, const __grid_constant__ ProjPlan plan,
-                                                                 const __grid_constant__ ProjSegments seg, double* __restrict__ coeff, int coeff_stride) {
-    __shared__ double s[16][32];
+// coeff[v*coeff_stride + user column] = sum over CTAs of partial[cta][v][slot-order column], the rows added in a fixed
+// order (reproducible): 32 lanes = 32 consecutive (v, column) elements; the block's 32 warps each add every 32nd row of
+// `partial` (coalesced, four loads in flight), then the 32 sums are added in order.
+__global__ void __launch_bounds__(1024) sh_project_reduce_kernel(const double* __restrict__ partial, int nrows, int nvec, const __grid_constant__ ProjPlan plan,
+                                                                  const __grid_constant__ ProjSegments seg, double* __restrict__ coeff, int coeff_stride) {
+    __shared__ double s[32][33];
     const int ncols = plan.ncols, ne = nvec * ncols;
     const int y = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int e = blockIdx.x * 32 + lane;
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
     if (e < ne) {
         int g = y;
-        for (; g + 48 < nwarps; g += 64) {
+        for (; g + 96 < nrows; g += 128) {
             a0 += partial[(int64_t)g * ne + e];
-            a1 += partial[(int64_t)(g + 16) * ne + e];
-            a2 += partial[(int64_t)(g + 32) * ne + e];
-            a3 += partial[(int64_t)(g + 48) * ne + e];
+            a1 += partial[(int64_t)(g + 32) * ne + e];
+            a2 += partial[(int64_t)(g + 64) * ne + e];
+            a3 += partial[(int64_t)(g + 96) * ne + e];
         }
-        for (; g < nwarps; g += 16) a0 += partial[(int64_t)g * ne + e];
+        for (; g < nrows; g += 32) a0 += partial[(int64_t)g * ne + e];
     }
     s[y][lane] = (a0 + a1) + (a2 + a3);
     __syncthreads();
     if (y == 0 && e < ne) {
         double t = 0.0;
-        for (int k = 0; k < 16; ++k) t += s[k][lane];
+        for (int k = 0; k < 32; ++k) t += s[k][lane];
         // slot-order column -> the caller's column
         const int v = e / ncols, c = e - v * ncols;
         int slot = 0;
@@ -1484,7 +1490,7 @@ void make_segments(const int* proj_l, const ProjPlan& plan, ProjSegments& seg) {
 int64_t project_workspace_bytes(int ncols, int nvec) {
     if (ncols < 0 || nvec < 0) return -1;
     const int64_t cols = ncols < PROJ_MAX_COLS ? ncols : PROJ_MAX_COLS, vecs = nvec < PROJ_NV ? nvec : PROJ_NV;
-    return (int64_t)sm_count() * PROJ_CTAS_PER_SM * 4 * vecs * cols * (int64_t)sizeof(double);
+    return (int64_t)sm_count() * PROJ_CTAS_PER_SM * vecs * cols * (int64_t)sizeof(double);   // one row per CTA of the largest grid
 }
 
 template <int LMAX>
@@ -1519,7 +1525,7 @@ int launch_project(const double* xyz, int64_t n, const double* radial, const Pro
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
     const int elems = nvec * plan.ncols;
-    sh_project_reduce_kernel<<<(elems + 31) / 32, 512, 0, st>>>(partial, (int)blocks * 4, nvec, plan, seg, coeff, coeff_stride);
+    sh_project_reduce_kernel<<<(elems + 31) / 32, 1024, 0, st>>>(partial, (int)blocks, nvec, plan, seg, coeff, coeff_stride);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     e = cudaGetLastError();
     return e == cudaSuccess ? SH_OK : cuda_fail(e);
