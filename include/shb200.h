@@ -167,7 +167,8 @@ enum {
     SH_TUNE_AOS_TILES_PER_WARP = 1, /* consecutive 32-point tiles one warp of the AoS kernels processes */
     SH_TUNE_PREFETCH_WINDOW_POINTS = 2, /* points per burst of the L2 input prefetch (default 262144); 1 = prefetch off */
     SH_TUNE_PROJ_AOS_MODE = 3,      /* sh_projectors AoS copy-out: 1 = warp copy, 2 = one bulk copy per row, 3 = one per tile (when possible) */
-    SH_TUNE_COUNT = 4
+    SH_TUNE_SOA_TMA = 4,            /* sh_real SoA through one TMA tensor store per 32-point tile: 0 = when possible (default), 1 = never */
+    SH_TUNE_COUNT = 5
 };
 int sh_set_tuning(int knob, int value);
 

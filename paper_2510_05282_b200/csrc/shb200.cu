@@ -14,6 +14,7 @@
 //
 // One thread evaluates one point; all (lmax+1)^2 values of a point are produced in ascending k by
 // straight-line code, so the store sinks below see compile-time offsets only.
+#include <cuda.h>   // CUtensorMap and the cuTensorMapEncodeTiled prototype only: the entry point is fetched through the runtime, libcuda is not linked
 #include <cuda_runtime.h>
 
 #include <atomic>
@@ -362,6 +363,56 @@ __global__ void __launch_bounds__(256) sh_soa_kernel(const TI* __restrict__ xyz,
     }
 }
 
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// a8, SoA through the TMA tensor unit (real fp64).  One warp = one 32-point tile; lane i stages value k of its point at
+// tile[k][i] (8-byte stores, 32 consecutive doubles per plane: conflict-free), and after a proxy fence lane 0 issues ONE
+// cp.async.bulk.tensor.2d store of the box {32 points, K planes} through a tensor map of `out` viewed as [K][n]: K rows of
+// 256 contiguous bytes, each two full 128-byte lines.  The LSU issues no global store at all (100 STG + their address
+// arithmetic per point in sh_soa_kernel), and points past n in a ragged last tile are clipped by the tensor unit.
+// One warp per CTA for the same reason as the AoS tile-bulk path (fence.proxy.async is CTA-scoped).
+#ifndef SHB200_SOA_TMA_WARPS
+#define SHB200_SOA_TMA_WARPS 4
+#endif
+// warps per CTA = 32-point groups per tile.  Longer rows are what the tile buys: 258 / 258 / 250 / 345 us for 1 / 2 / 4 / 8 warps
+// (rows of 256 B .. 2 KB; 8 warps = one 205 KB tile per SM, nothing overlaps) on the 128^3 grid at lmax = 9.
+// (The fp32 variant gains nothing from it -- 255 vs 257 us on 2^22 points -- and stays on sh_soa_pair_kernel.)
+constexpr int SOA_TMA_WARPS = SHB200_SOA_TMA_WARPS;
+
+template <int PTS>
+struct TileSink {
+    double* col;   // tile + this thread's point
+    template <int K> __device__ __forceinline__ void put1(double v) { col[K * PTS] = v; }
+    template <int L> __device__ __forceinline__ void end_l() {}
+    template <int L> __device__ __forceinline__ void polar(const double (&)[L + 1]) {}
+};
+
+template <int LMAX, int WARPS>
+__global__ void __launch_bounds__(32 * WARPS) sh_soa_tma_kernel(const double* __restrict__ xyz, int64_t n, const __grid_constant__ CUtensorMap tmap, int coords,
+                                                                 InputPrefetch pf) {
+    constexpr int PTS = 32 * WARPS;
+    extern __shared__ __align__(128) unsigned char smem_tile[];
+    prefetch_input_window(xyz, n * 24, (int64_t)PTS * 24, pf);
+    double* tile = reinterpret_cast<double*>(smem_tile);
+    const int64_t base = (int64_t)blockIdx.x * PTS, i = base + threadIdx.x;
+    if (i < n) {
+        RawPoint<double> pt;
+        pt.load(xyz, i);
+        TileSink<PTS> sink{tile + threadIdx.x};
+        evaluate<KIND_REAL, LMAX, double>(pt.unit(coords), sink);
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // every thread: its staging stores -> async proxy
+    if constexpr (WARPS == 1) __syncwarp();
+    else __syncthreads();
+    if (threadIdx.x == 0) {
+        asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];" ::"l"(&tmap), "r"((int)base), "r"(0),
+                     "r"(smem_u32(tile))
+                     : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory is released when the CTA exits
+    }
+}
+
 // fp32 SoA, two ADJACENT points (2j, 2j+1) per thread: 8-byte stores (a warp store covers 256 B of a plane),
 // half the store and address instructions per point, packed-fp32 arithmetic.  Needs even n and 8-byte aligned out.
 struct SoAPairSink {
@@ -547,8 +598,6 @@ struct Segments {
         return max_len() | 1;
     }
 };
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 template <int KIND, int LMAX, typename T, int CAP, int MODE>
 struct RowSink {
@@ -895,6 +944,13 @@ __global__ void __launch_bounds__(128) sh_proj_aos_kernel(const double* __restri
 // Running sums are kept in the order of production ("slot order"); at the end a CTA adds its four warps in a fixed order
 // and writes one row of `partial` [cta][nvec][ncols]; sh_project_reduce_kernel adds the rows in a fixed order and
 // scatters to the caller's column order.
+#ifndef SHB200_PROJ_CTAS_NV1
+#define SHB200_PROJ_CTAS_NV1 4
+#endif
+#ifndef SHB200_PROJ_CTAS_NV4
+#define SHB200_PROJ_CTAS_NV4 3
+#endif
+constexpr int PROJ_CTAS_NV1 = SHB200_PROJ_CTAS_NV1, PROJ_CTAS_NV4 = SHB200_PROJ_CTAS_NV4;   // resident CTAs per SM (__launch_bounds__): register budget
 constexpr int PROJ_NV = 4;          // weight vectors contracted per launch
 constexpr int PROJ_MAX_COLS = 128;  // columns per launch (whole channels); wider channel lists run as several launches
 constexpr int PROJ_SEG_PITCH = 34;  // doubles between consecutive columns of the transposed segment tile
@@ -962,7 +1018,7 @@ struct ProjectSink {
 };
 
 template <int LMAX, int NV>
-__global__ void __launch_bounds__(128, NV == 1 ? 4 : 3) sh_project_kernel(const double* __restrict__ xyz, int64_t n, const double* __restrict__ radial,
+__global__ void __launch_bounds__(128, NV == 1 ? PROJ_CTAS_NV1 : PROJ_CTAS_NV4) sh_project_kernel(const double* __restrict__ xyz, int64_t n, const double* __restrict__ radial,
                                                                           const __grid_constant__ ProjPlan plan, const __grid_constant__ ProjSegments seg,
                                                                           const double* __restrict__ w, int nvec, double* __restrict__ partial) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -1111,6 +1167,54 @@ int launch_soa(const TI* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
     return e == cudaSuccess ? SH_OK : cuda_fail(e);
 }
 
+inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point lookup (no link against libcuda); nullptr if unavailable
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                   const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled() {
+    static EncodeTiledFn fn = [] {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) p = nullptr;
+        return reinterpret_cast<EncodeTiledFn>(p);
+    }();
+    return fn;
+}
+
+// SoA through the tensor unit: `out` as a 2-D tensor [K][n] of fp64 (row pitch 8n bytes must be a multiple of 16: n even),
+// box {points per tile, K}.  Returns SH_ERR_ALIGNMENT when this launch cannot use the path (the caller then takes sh_soa_kernel).
+template <int LMAX>
+int launch_soa_tma(const double* xyz, int64_t n, double* out, int coords, cudaStream_t st) {
+    constexpr int K = (LMAX + 1) * (LMAX + 1);
+    constexpr int PTS = 32 * SOA_TMA_WARPS;
+    EncodeTiledFn enc = encode_tiled();
+    if (!enc || (n & 1) || n < PTS || n > 0x7fffff00LL || !aligned(out, 16)) return SH_ERR_ALIGNMENT;
+    CUtensorMap tmap;
+    const cuuint64_t gdim[2] = {(cuuint64_t)n, (cuuint64_t)K};
+    const cuuint64_t gstride[1] = {(cuuint64_t)n * sizeof(double)};
+    const cuuint32_t box[2] = {PTS, (cuuint32_t)K}, estride[2] = {1, 1};
+    if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, out, gdim, gstride, box, estride, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+            CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return SH_ERR_ALIGNMENT;
+    const int64_t blocks = (n + PTS - 1) / PTS;
+    constexpr size_t smem = (size_t)K * PTS * sizeof(double);
+    static_assert(smem <= 227 * 1024, "tile exceeds shared memory");
+    auto kern = sh_soa_tma_kernel<LMAX, SOA_TMA_WARPS>;
+    if constexpr (smem > 48 * 1024) {
+        static bool opted_in = false;
+        if (!opted_in) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return cuda_fail(e);
+            opted_in = true;
+        }
+    }
+    kern<<<(unsigned)blocks, PTS, smem, st>>>(xyz, n, tmap, coords, prefetch_plan(n, PTS));
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? SH_OK : cuda_fail(e);
+}
+
 // staging capacity per row, in scalars: whole rows for real (800 B at lmax = 9) and complex (1600 B);
 // spinor rows (6400 B) are staged in groups of l-blocks of at most 1600 B
 template <int KIND, int LMAX>
@@ -1184,8 +1288,6 @@ int launch_soa_pair(const float* xyz, int64_t n, float* out, int coords, cudaStr
     return e == cudaSuccess ? SH_OK : cuda_fail(e);
 }
 
-inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
-
 template <int KIND, int LMAX, typename T, typename TI>
 int dispatch_lmax(const TI* xyz, int64_t n, T* out, int layout, int path, int coords, cudaStream_t st) {
     constexpr int SP = scalars_per_point(KIND, LMAX);
@@ -1200,6 +1302,13 @@ int dispatch_lmax(const TI* xyz, int64_t n, T* out, int layout, int path, int co
     if (layout == SH_LAYOUT_SOA) {
         if (path == SH_STORE_BULK) return SH_ERR_ALIGNMENT;   // bulk path is AoS only
         constexpr int ES = elem_scalars(KIND);
+        if constexpr (KIND == KIND_REAL && std::is_same<T, double>::value) {
+            // one tensor-map store per 128-point tile where `out` allows it (16-byte aligned, even n)
+            if (path == SH_STORE_AUTO && tuned(SH_TUNE_SOA_TMA, 0) != 1) {
+                const int rc = launch_soa_tma<LMAX>(reinterpret_cast<const double*>(xyz), n, reinterpret_cast<double*>(out), coords, st);
+                if (rc != SH_ERR_ALIGNMENT) return rc;
+            }
+        }
         if constexpr (F32) {
             // two adjacent points per thread (packed fp32, 8-byte stores) when every plane keeps 8-byte alignment
             if (n >= 2 && n % 2 == 0 && aligned(out, 8) && aligned(xyz, 8) && path != SH_STORE_DIRECT)
@@ -1399,7 +1508,7 @@ int check_projector_args(const double* xyz, int64_t n, int nproj, const int* pro
     return SH_OK;
 }
 
-constexpr int PROJ_CTAS_PER_SM = 4;   // grid cap of sh_project_kernel: the machine filled once (what the workspace is sized for)
+constexpr int PROJ_CTAS_PER_SM = PROJ_CTAS_NV1 > PROJ_CTAS_NV4 ? PROJ_CTAS_NV1 : PROJ_CTAS_NV4;   // grid cap of sh_project_kernel: the machine filled once (what the workspace is sized for)
 
 template <int LMAX>
 int launch_proj_aos(const double* xyz, int64_t n, const double* radial, const ProjPlan& plan, double* out, cudaStream_t st) {
@@ -1463,7 +1572,10 @@ int run_projectors(const double* xyz, int64_t n, int nproj, const int* proj_l, c
     switch (lmax) {
 #define SH_CASE(L) case L: return layout_bits == SH_LAYOUT_SOA ? launch_proj_soa<L>(xyz, n, radial, plan, out, st) \
                                                              : launch_proj_aos<L>(xyz, n, radial, plan, out, st);
-        SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(3) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8) SH_CASE(9)
+#ifndef SHB200_DEV_ONLY_LMAX9
+        SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8)
+#endif
+        SH_CASE(3) SH_CASE(9)
 #undef SH_CASE
     }
     return SH_ERR_PROJECTOR;
@@ -1498,7 +1610,7 @@ int launch_project(const double* xyz, int64_t n, const double* radial, const Pro
                    double* partial, double* coeff, int coeff_stride, cudaStream_t st) {
     const int64_t ntiles = (n + 31) / 32;
     int64_t blocks = (ntiles + 3) / 4;
-    const int64_t cap = (int64_t)sm_count() * (nvec == 1 ? PROJ_CTAS_PER_SM : PROJ_CTAS_PER_SM - 1);   // resident CTAs per SM (__launch_bounds__)
+    const int64_t cap = (int64_t)sm_count() * (nvec == 1 ? PROJ_CTAS_NV1 : PROJ_CTAS_NV4);   // resident CTAs per SM (__launch_bounds__)
     if (blocks > cap) blocks = cap;
     // per warp: segment tile, running sums, (weights,) and the radial values of every slot: 38 / 54 KB + 1 KB per slot per CTA
     const size_t slots_bytes = (size_t)4 * 32 * plan.first[shgen::LMAX_CAP + 1] * sizeof(double);
@@ -1559,7 +1671,10 @@ int run_project(const double* xyz, int64_t n, int nproj, const int* proj_l, cons
             const int nv = nvec - v0 < PROJ_NV ? nvec - v0 : PROJ_NV;
             switch (lmax) {
 #define SH_CASE(L) case L: rc = launch_project<L>(xyz, n, radial, plan, seg, w + (int64_t)v0 * n, nv, partial, coeff + (int64_t)v0 * ncols + c0, ncols, st); break;
-                SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(3) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8) SH_CASE(9)
+#ifndef SHB200_DEV_ONLY_LMAX9
+                SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8)
+#endif
+                SH_CASE(3) SH_CASE(9)
 #undef SH_CASE
             }
             if (rc != SH_OK) return rc;

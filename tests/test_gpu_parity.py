@@ -110,6 +110,27 @@ def test_bulk_request_matches_and_is_refused_when_impossible(sh, oracle_mod, cub
         gpu_eval(sh, "real", cube_points, 9, "aos", "bulk", misalign=1)
 
 
+@pytest.mark.parametrize("lmax", range(10))
+def test_soa_tensor_store_and_lsu_store_paths(sh, oracle_mod, lmax):
+    """sh_real SoA has two store mechanisms: one TMA tensor store per 128-point tile (even n >= 128, 16-byte aligned out)
+    and per-thread streaming stores (everything else, or `soa_tma` = 1).  Both against the oracle and against each other
+    (same arithmetic: bit-identical), at sizes with full tiles, a ragged last tile and fewer points than one tile."""
+    rng = np.random.default_rng(300 + lmax)
+    for n in (126, 128, 130, 1000, 4098):
+        pts = rng.uniform(-2, 2, (n, 3))
+        pts[0] = 0.0                     # r = 0 convention
+        pts[1] = (0.0, 0.0, -1.5)        # pole
+        want = oracle_mod.real(pts, lmax)
+        got_tma = gpu_eval(sh, "real", pts, lmax, "soa")
+        sh.set_tuning("soa_tma", 1)
+        try:
+            got_lsu = gpu_eval(sh, "real", pts, lmax, "soa")
+        finally:
+            sh.set_tuning("soa_tma", 0)
+        assert max_err(got_tma, want) <= TOL64 and max_err(got_lsu, want) <= TOL64, n
+        assert np.array_equal(got_tma, got_lsu), n
+
+
 @pytest.mark.parametrize("kind", ["real", "complex", "spinor"])
 @pytest.mark.parametrize("layout", ["soa", "aos"])
 def test_misaligned_out_and_odd_n_fall_back(sh, oracle_mod, kind, layout):
