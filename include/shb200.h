@@ -55,7 +55,9 @@ enum {
  * alignment allows.  A request the alignment does not allow returns SH_ERR_ALIGNMENT.  Results are identical
  * on every path (same arithmetic, different store mechanism). */
 enum {
-    SH_STORE_AUTO   = 0 << 8,
+    SH_STORE_AUTO   = 0 << 8, /* sh_real SoA with even n >= 128 and a 16-byte aligned out: tiles of 128 points staged in shared memory and
+                                 written by one TMA tensor store each (cp.async.bulk.tensor.2d through a tensor map of out as [K][n]);
+                                 AoS with a 16-byte aligned out: SH_STORE_BULK; everything else: SH_STORE_DIRECT */
     SH_STORE_DIRECT = 1 << 8, /* per-thread st.global.cs; SoA: coalesced planes; AoS: smem transpose + coalesced stores */
     SH_STORE_BULK   = 2 << 8  /* AoS only, needs a 16-byte aligned out: rows staged in shared memory, written by TMA bulk copies
                                  (cp.async.bulk): one copy per 32-point tile where the layout allows, else one per row */
@@ -168,7 +170,9 @@ enum {
     SH_TUNE_PREFETCH_WINDOW_POINTS = 2, /* points per burst of the L2 input prefetch (default 262144); 1 = prefetch off */
     SH_TUNE_PROJ_AOS_MODE = 3,      /* sh_projectors AoS copy-out: 1 = warp copy, 2 = one bulk copy per row, 3 = one per tile (when possible) */
     SH_TUNE_SOA_TMA = 4,            /* sh_real SoA through one TMA tensor store per 32-point tile: 0 = when possible (default), 1 = never */
-    SH_TUNE_COUNT = 5
+    SH_TUNE_PROJECT_FORM = 5,       /* sh_project polynomials: 0 = the factorized forms of every other call (default); 1 = Horner in z^2 for the
+                                       polar factors and (x + iy)^m by recurrence: ~35 % fewer FP64 instructions, same tolerance */
+    SH_TUNE_COUNT = 6
 };
 int sh_set_tuning(int knob, int value);
 

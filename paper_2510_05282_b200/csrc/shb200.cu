@@ -173,14 +173,28 @@ __device__ __forceinline__ void prefetch_input_window(const void* in, int64_t to
 // ------------------------------------------------------------------------------------------------
 // a3-a7: evaluators.  Sink interface: put1<K>(v) real element K; put2<K>(re, im) complex element K;
 // put4<S>(ur, ui, dr, di) spinor element S; end_l<L>() after the last element of block l.
-template <int LMAX, typename T>
+// REC = false: the factorized forms (root-pair products, Eq. 16).  REC = true: C_m + i S_m = (C_{m-1} + i S_{m-1})(x + i y),
+// four instructions per m instead of ~17; used only by the FP64-bound projection when its fast form is requested.
+template <int LMAX, typename T, bool REC = false>
 struct Azim {
     T C[LMAX + 1], S[LMAX + 1];
     __device__ __forceinline__ Azim(T x, T y) {
-        static_for<0, LMAX + 1>([&](auto mc) {
-            constexpr int M = decltype(mc)::value;
-            shgen::Azimuthal<M, T>::eval(x, y, C[M], S[M]);
-        });
+        if constexpr (REC) {
+            C[0] = T(1); S[0] = T(0);
+            static_for<1, LMAX + 1>([&](auto mc) {
+                constexpr int M = decltype(mc)::value;
+                if constexpr (M == 1) { C[1] = x; S[1] = y; }
+                else {
+                    C[M] = C[M - 1] * x - S[M - 1] * y;
+                    S[M] = C[M - 1] * y + S[M - 1] * x;
+                }
+            });
+        } else {
+            static_for<0, LMAX + 1>([&](auto mc) {
+                constexpr int M = decltype(mc)::value;
+                shgen::Azimuthal<M, T>::eval(x, y, C[M], S[M]);
+            });
+        }
     }
 };
 
@@ -805,9 +819,12 @@ __device__ __forceinline__ void stage_radial(const RadialPos& pos, const double*
 }
 
 // the real harmonics of block l in ascending m (a3-a5), handed to the sink one block at a time
-template <int LMAX, class Sink>
+// FAST: Horner-in-z^2 polar factors and the azimuthal recurrence instead of the factorized forms -- ~35 % fewer FP64
+// instructions, accuracy still two orders inside the tolerance; sh_project only, on request.
+template <int LMAX, bool FAST = false, class Sink>
 __device__ __forceinline__ void eval_projector_blocks(const UnitVec& u, const ProjPlan& plan, Sink& sink) {
-    const Azim<LMAX, double> az(u.x, u.y);
+    const Azim<LMAX, double, FAST> az(u.x, u.y);
+    [[maybe_unused]] const double z2 = u.z * u.z;
     static_for<0, LMAX + 1>([&](auto lc) {
         constexpr int L = decltype(lc)::value;
         if (plan.first[L] != plan.first[L + 1]) {
@@ -815,7 +832,9 @@ __device__ __forceinline__ void eval_projector_blocks(const UnitVec& u, const Pr
             static_for<0, L + 1>([&](auto mc) {
                 constexpr int M = decltype(mc)::value;
                 constexpr double A = shgen::A_REAL[L][M];
-                double q = A * shgen::Polar<L, M, double>::eval(u.z);
+                double q;
+                if constexpr (FAST) q = A * shgen::PolarHorner<L, M, double>::eval(u.z, z2);
+                else q = A * shgen::Polar<L, M, double>::eval(u.z);
                 if constexpr (M == 0) {
                     if constexpr (L > 0 && L % 2 == 0) q = zero_where(u.origin, q);   // P_l(0) != 0: the r = 0 convention needs it
                     blk[L] = q;
@@ -1017,7 +1036,7 @@ struct ProjectSink {
     }
 };
 
-template <int LMAX, int NV>
+template <int LMAX, int NV, bool FAST>
 __global__ void __launch_bounds__(128, NV == 1 ? PROJ_CTAS_NV1 : PROJ_CTAS_NV4) sh_project_kernel(const double* __restrict__ xyz, int64_t n, const double* __restrict__ radial,
                                                                           const __grid_constant__ ProjPlan plan, const __grid_constant__ ProjSegments seg,
                                                                           const double* __restrict__ w, int nvec, double* __restrict__ partial) {
@@ -1060,7 +1079,7 @@ __global__ void __launch_bounds__(128, NV == 1 ? PROJ_CTAS_NV1 : PROJ_CTAS_NV4) 
         const RadialPos pos(cur.x, cur.y, cur.z, plan);
         stage_radial(pos, radial, plan, s_fs, lane, NV == 1 ? cur.w[0] : 1.0);   // only this lane reads its column back
         ProjectSink<NV> sink{s_tile, s_sums, s_wt, s_fs + lane, plan, seg, lane};
-        eval_projector_blocks<LMAX>(normalize(cur.x, cur.y, cur.z), plan, sink);
+        eval_projector_blocks<LMAX, FAST>(normalize(cur.x, cur.y, cur.z), plan, sink);
         cur = nxt;
     }
     // the CTA's four warps are added in a fixed order: one row of `partial` per CTA
@@ -1615,24 +1634,26 @@ int launch_project(const double* xyz, int64_t n, const double* radial, const Pro
     // per warp: segment tile, running sums, (weights,) and the radial values of every slot: 38 / 54 KB + 1 KB per slot per CTA
     const size_t slots_bytes = (size_t)4 * 32 * plan.first[shgen::LMAX_CAP + 1] * sizeof(double);
     constexpr size_t smem_max = (size_t)4 * (project_smem_doubles_per_warp<PROJ_NV>() + 32 * SH_MAX_PROJ) * sizeof(double);   // 86 KB
-    static bool opted_in[2] = {false, false};
+    const bool fast = tuned(SH_TUNE_PROJECT_FORM, 0) == 1;   // Horner / recurrence forms instead of the factorized ones
+    auto launch = [&](auto kern, size_t warp_doubles, bool& opted_in) -> int {
+        if (!opted_in) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
+            if (e != cudaSuccess) return cuda_fail(e);
+            opted_in = true;
+        }
+        kern<<<(unsigned)blocks, 128, (size_t)4 * warp_doubles * sizeof(double) + slots_bytes, st>>>(xyz, n, radial, plan, seg, w, nvec, partial);
+        return SH_OK;
+    };
+    static bool opted_in[4] = {false, false, false, false};
+    int rc;
     if (nvec == 1) {
-        const size_t smem = (size_t)4 * project_smem_doubles_per_warp<1>() * sizeof(double) + slots_bytes;
-        if (!opted_in[0]) {
-            cudaError_t e = cudaFuncSetAttribute(sh_project_kernel<LMAX, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
-            if (e != cudaSuccess) return cuda_fail(e);
-            opted_in[0] = true;
-        }
-        sh_project_kernel<LMAX, 1><<<(unsigned)blocks, 128, smem, st>>>(xyz, n, radial, plan, seg, w, nvec, partial);
+        rc = fast ? launch(sh_project_kernel<LMAX, 1, true>, project_smem_doubles_per_warp<1>(), opted_in[1])
+                  : launch(sh_project_kernel<LMAX, 1, false>, project_smem_doubles_per_warp<1>(), opted_in[0]);
     } else {
-        const size_t smem = (size_t)4 * project_smem_doubles_per_warp<PROJ_NV>() * sizeof(double) + slots_bytes;
-        if (!opted_in[1]) {
-            cudaError_t e = cudaFuncSetAttribute(sh_project_kernel<LMAX, PROJ_NV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
-            if (e != cudaSuccess) return cuda_fail(e);
-            opted_in[1] = true;
-        }
-        sh_project_kernel<LMAX, PROJ_NV><<<(unsigned)blocks, 128, smem, st>>>(xyz, n, radial, plan, seg, w, nvec, partial);
+        rc = fast ? launch(sh_project_kernel<LMAX, PROJ_NV, true>, project_smem_doubles_per_warp<PROJ_NV>(), opted_in[3])
+                  : launch(sh_project_kernel<LMAX, PROJ_NV, false>, project_smem_doubles_per_warp<PROJ_NV>(), opted_in[2]);
     }
+    if (rc != SH_OK) return rc;
     g_launches.fetch_add(1, std::memory_order_relaxed);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);

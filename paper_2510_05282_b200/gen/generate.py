@@ -94,6 +94,14 @@ def q_factorization(l: int, m: int):
     return lead, par, roots
 
 
+def q_monic_in_z2(l: int, m: int) -> list[Fraction]:
+    """Qhat_l^m / z^par as a MONIC polynomial in w = z^2: exact coefficients, ascending powers (last one is 1)."""
+    c = q_poly(l, m)
+    deg = l - m
+    par = deg % 2
+    return [c[par + 2 * i] / c[deg] for i in range(deg // 2 + 1)]
+
+
 def K(l: int, m: int):
     return mp.sqrt(mp.mpf(2 * l + 1) / (4 * mp.pi) * mp.mpf(factorial(l - m)) / mp.mpf(factorial(l + m)))
 
@@ -147,6 +155,13 @@ def self_check():
                 assert abs(val - ref) < mp.mpf(10) ** -25 * max(1, abs(ref)), ("polar/mpmath", l, m)
                 exact = sum((mp.mpf(c.numerator) / c.denominator) * z**k for k, c in enumerate(q_poly(l, m)))
                 assert abs(val - exact) < tol * max(1, abs(exact)), ("polar/exact", l, m)
+                # the Horner form in z^2 emitted for the FP64-bound consumer (PolarHorner)
+                w = q_monic_in_z2(l, m)
+                acc = mp.mpf(1)
+                for cf in reversed(w[:-1]):
+                    acc = acc * z * z + mp.mpf(cf.numerator) / cf.denominator
+                hv = mp.mpf(lead.numerator) / lead.denominator * z**par * acc
+                assert abs(hv - exact) < tol * max(1, abs(exact)), ("polar/horner", l, m)
 
 
 # ----------------------------------------------------------------------------- recurrence extension, l > 9
@@ -246,6 +261,24 @@ def emit() -> str:
             body = " * ".join(terms) if terms else "T(1)"
             arg = "T z" if terms else "T"
             w(f"template <typename T> struct Polar<{l}, {m}, T> {{ static SHGEN_FN T eval({arg}) {{ return {body}; }} }};")
+    w("")
+    w("// ---- the same polar factors in Horner form in t = z^2 (the paper's fallback form, PAPER.md line 124), monic: ----")
+    w("// Qhat_l^m(z) = z^((l-m)%2) (((t + c_{k-1}) t + c_{k-2}) t + ... + c_0).  One FMA per root pair instead of four")
+    w("// instructions; not used by the sh_* calls (PAPER.md lines 93, 122: accuracy), offered to the FP64-bound projection.")
+    w("template <int L, int M, typename T> struct PolarHorner;")
+    for l in range(LMAX + 1):
+        for m in range(l + 1):
+            cs = q_monic_in_z2(l, m)
+            par = (l - m) % 2
+            body = None
+            for cf in reversed(cs[:-1]):
+                c_lit = "T(" + dlit(mp.mpf(cf.numerator) / cf.denominator) + ")"
+                body = f"(t + {c_lit})" if body is None else f"({body} * t + {c_lit})"
+            if body is None:
+                body = "z" if par else "T(1)"
+            elif par:
+                body = f"z * {body}"
+            w(f"template <typename T> struct PolarHorner<{l}, {m}, T> {{ static SHGEN_FN T eval(T z, T t) {{ (void)z; (void)t; return {body}; }} }};")
     w("")
     w("// ---- constants (fp64; cast at the point of use) ----")
     w("// A_REAL[l][m]: R_l^0 = A Qhat,  R_l^{+-m} = A Qhat {C_m, S_m}   (A = sqrt2 K_l^m lead_lm, m > 0)")

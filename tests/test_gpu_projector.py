@@ -136,6 +136,53 @@ def test_aos_store_modes(sh, oracle_mod, proj_l):
                 assert np.abs(got - want).max() <= TOL * max(1.0, np.abs(tab).max()), (n, mis, mode)
 
 
+@pytest.mark.parametrize("form", [0, 1])
+def test_project_polynomial_forms_value_by_value(sh, oracle_mod, form):
+    """sh_project has two polynomial forms (`project_form` knob): the factorized ones (0) and Horner in z^2 + the
+    (x + iy)^m recurrence (1).  One-hot weight vectors turn the projection into the per-point values (every other term
+    of the sum is an exact 0), so each form is checked VALUE BY VALUE against the oracle at the fp64 tolerance: random
+    directions, points within 1e-6 of the poles and the axes, the origin, points beyond the table."""
+    rng = np.random.default_rng(17)
+    n = 96
+    g = rng.standard_normal((n, 3))
+    g[:24, :2] *= 1e-6          # near the poles
+    g[24:36, 2] *= 1e-7         # near the equator (z ~ 0: the odd polynomials' zero)
+    g[36:44, 1] *= 1e-9         # near the x axis
+    pts = g / np.linalg.norm(g, axis=1)[:, None] * rng.uniform(0.05, 3.1, n)[:, None]
+    pts[44] = 0.0
+    pts[45] = (0.0, 0.0, -1.25)
+    proj_l = [9, 0, 8, 1, 7, 2, 6, 3, 5, 4, 9]
+    nr, dr = 31, 0.1
+    tab = rng.standard_normal((len(proj_l), nr))
+    tab[:, -1] = 0.0
+    want = oracle_mod.projectors(pts, proj_l, tab, dr)          # [n][ncols]
+    sh.set_tuning("project_form", form)
+    try:
+        got = gpu_project(sh, pts, proj_l, tab, dr, np.eye(n))   # coeff[v][col] = beta_col(point v)
+    finally:
+        sh.set_tuning("project_form", 0)
+    err = np.abs(got - want).max()
+    print(f"project_form {form}: max |beta_gpu - beta_oracle| = {err:.2e}")
+    assert err <= TOL * max(1.0, np.abs(tab).max())
+
+
+@pytest.mark.parametrize("nvec", [1, 4])
+def test_project_fast_forms_full_grid(sh, oracle_mod, nvec):
+    """The Horner / recurrence forms on the bench's FP64-bound workload (128^3 grid, 100 columns) against the oracle's sum."""
+    from paper_2510_05282_b200 import inputs
+
+    pts = inputs.config3_full_grid()
+    proj_l, tab, dr = inputs.projector_channels(lmax=9, per_l=1, cutoff=6.0, dr=0.02)
+    w = inputs.wave_weights(len(pts), nvec, seed=8, volume_element=(12.0 / 128) ** 3)
+    coeff, abs_sum = oracle_mod.project(pts, proj_l, tab, dr, w)
+    sh.set_tuning("project_form", 1)
+    try:
+        got = gpu_project(sh, pts, proj_l, tab, dr, w)
+    finally:
+        sh.set_tuning("project_form", 0)
+    check_project(got, coeff, abs_sum)
+
+
 def test_many_channels_wide_rows(sh, oracle_mod):
     """32 channels of l = 9: 608 columns -- the AoS tile is 156 KB (one warp per CTA) and the projection runs as five
     launches of at most 128 columns."""
