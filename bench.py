@@ -356,7 +356,10 @@ def run_ours(args):
     import paper_2510_05282_b200 as sh
     from paper_2510_05282_b200.dist import env_world, max_over_ranks
 
-    sh.load()  # no fallback: fails here if libshb200.so is missing
+    from paper_2510_05282_b200 import build as _build
+
+    _build.ensure_built()  # compiles only if the in-tree library is absent
+    sh.load()  # no fallback: fails here if libshb200.so cannot be loaded
     rank, local, world = env_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the CUDA path has no CPU fallback)")

@@ -46,5 +46,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def ensure_built() -> str:
+    """Compile only if libshb200.so is absent (a fresh checkout on a box that has nvcc).  Never a fallback: the result is
+    the same CUDA library, and binding.load() still raises if it cannot be produced."""
+    return LIB if os.path.exists(LIB) else build(force=True)
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -22,7 +22,9 @@ def sh():
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     import paper_2510_05282_b200 as pkg
+    from paper_2510_05282_b200 import build
 
+    build.ensure_built()   # compiles only if the in-tree library is absent
     pkg.load()
     return pkg
 
