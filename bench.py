@@ -45,11 +45,17 @@ def measured_peak():
 
 
 def ncu_traffic(kernel_key: str):
-    """Per-launch DRAM bytes of the dominant kernel from the committed ncu summary, or None."""
+    """Per-launch DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel from the committed ncu
+    summary profiles/ncu_traffic.csv (see profiles/r1_launches.md for the commands), or None."""
     try:
-        return json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))[kernel_key]["dram_bytes_per_launch"]
+        import csv
+
+        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "ncu_traffic.csv"))):
+            if row["kernel"] == kernel_key:
+                return float(row["dram_bytes_per_launch"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
@@ -122,9 +128,20 @@ def cpu_baseline(pts, target_seconds=12.0):
     t0 = time.perf_counter()
     oracle.real(pts[:m], LMAX)
     dt = time.perf_counter() - t0
+    cores = oracle.threads_used()
+    # one thread as well (comparable with the paper's single-core figures), on a smaller prefix
+    m1 = max(1 << 12, m // (4 * max(cores, 1)))
+    oracle.set_threads(1)
+    try:
+        t0 = time.perf_counter()
+        oracle.real(pts[:m1], LMAX)
+        dt1 = time.perf_counter() - t0
+    finally:
+        oracle.set_threads(0)
     return {
-        "value": m * K / dt / 1e9, "unit": UNIT, "cores": oracle.threads_used(), "kind": "oracle",
+        "value": m * K / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
         "sample": f"first {m} points of the 128^3 grid, lmax=9 real, long double, one evaluation, {dt:.2f} s",
+        "value_one_thread": m1 * K / dt1 / 1e9, "sample_one_thread": f"first {m1} points, {dt1:.2f} s",
     }
 
 
