@@ -1,6 +1,6 @@
 """paper_2510_05282_b200: batched real / complex / spinor spherical harmonics (l <= 9) on one B200.
 
-The product is the C-ABI library libshb200.so (include/shb200.h, csrc/shb200.cu); this package holds the
+The product is the C-ABI library libshb200.so (include/shb200.h, csrc/*.cu); this package holds the
 build step, the build-time formula generator, a thin ctypes binding and the seeded workload generators.
 """
 from .binding import (  # noqa: F401

@@ -1,4 +1,5 @@
-"""Build step: run the generator, then compile csrc/shb200.cu for sm_100a into libshb200.so (in-tree).
+"""Build step: run the generator, then compile csrc/*.cu for sm_100a (one nvcc per translation unit, in parallel) and
+link them into libshb200.so (in-tree).
 
     python -m paper_2510_05282_b200.build [--force]
 
@@ -13,11 +14,13 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libshb200.so")
-SOURCES = ["shb200.cu"]
+# one harmonic kind per unit (they compile in parallel), the l > 9 extension, the fused projector consumer, shared host state
+SOURCES = ["sh_real.cu", "sh_complex.cu", "sh_spinor.cu", "sh_real_f32.cu", "sh_ext.cu", "sh_projector.cu", "sh_abi.cu"]
+HEADERS = ["sh_core.cuh", "sh_store.cuh", "sh_generated.cuh"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17", "--expt-relaxed-constexpr",
-    "-Xcompiler", "-fPIC", "-shared",
+    "-Xcompiler", "-fPIC",
 ]
 
 
@@ -34,14 +37,34 @@ def generate() -> str:
     return g.main(["generate.py", os.path.join(CSRC, "sh_generated.cuh")])
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    gen = generate()
-    deps = [gen, os.path.join(HERE, "..", "include", "shb200.h")] + [os.path.join(CSRC, s) for s in SOURCES]
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
+def build(force: bool = False, verbose: bool = False, extra_flags: tuple = ()) -> str:
+    """Objects go to csrc/build/ (git-ignored); a unit is recompiled when it, a header or the flags changed."""
+    generate()
+    common = [os.path.join(HERE, "..", "include", "shb200.h")] + [os.path.join(CSRC, h) for h in HEADERS]
+    flags = NVCC_FLAGS + list(extra_flags) + (["-Xptxas", "-v"] if verbose else [])
+    objdir = os.path.join(CSRC, "build")
+    os.makedirs(objdir, exist_ok=True)
+    stamp = os.path.join(objdir, "flags.txt")
+    if not os.path.exists(stamp) or open(stamp).read() != " ".join(flags):
+        force = True
+    jobs = []
+    for s in SOURCES:
+        src, obj = os.path.join(CSRC, s), os.path.join(objdir, s[:-3] + ".o")
+        if force or not os.path.exists(obj) or any(os.path.getmtime(obj) < os.path.getmtime(d) for d in [src] + common):
+            jobs.append((s, obj, subprocess.Popen([_nvcc()] + flags + ["-c", src, "-o", obj])))
+    failed = [s for s, _, proc in jobs if proc.wait() != 0]
+    if failed:
+        for s, obj, _ in jobs:
+            if s in failed and os.path.exists(obj):
+                os.remove(obj)
+        raise RuntimeError("nvcc failed for " + ", ".join(failed))
+    with open(stamp, "w") as f:
+        f.write(" ".join(flags))
+    objs = [os.path.join(objdir, s[:-3] + ".o") for s in SOURCES]
+    if not jobs and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(o) for o in objs):
         return LIB
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
-    subprocess.check_call(cmd)
+    subprocess.check_call([_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp] + objs)
     os.replace(tmp, LIB)
     return LIB
 
@@ -53,4 +76,5 @@ def ensure_built() -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    # extra nvcc flags (e.g. -DSHB200_DEV_ONLY_LMAX9 for development builds) pass through
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, extra_flags=tuple(a for a in sys.argv[1:] if a.startswith("-D"))))
