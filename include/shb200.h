@@ -172,7 +172,8 @@ enum {
     SH_TUNE_SOA_TMA = 4,            /* sh_real SoA through one TMA tensor store per 32-point tile: 0 = when possible (default), 1 = never */
     SH_TUNE_PROJECT_FORM = 5,       /* sh_project polynomials: 0 = the factorized forms of every other call (default); 1 = Horner in z^2 for the
                                        polar factors and (x + iy)^m by recurrence: ~35 % fewer FP64 instructions, same tolerance */
-    SH_TUNE_COUNT = 6
+    SH_TUNE_PROJ_AOS_SPLIT = 6,     /* sh_projectors AoS, lmax >= 4: warps that share one 32-point tile, each evaluating part of the l-blocks: 1, 2 (default) or 4 */
+    SH_TUNE_COUNT = 7
 };
 int sh_set_tuning(int knob, int value);
 

@@ -49,32 +49,52 @@ __device__ __forceinline__ void stage_radial(const RadialPos& pos, const double*
     for (int s = 0; s < nslots; ++s) fs[s * 32 + lane] = pos.f(radial, plan.nr, plan.chan[s]) * scale;
 }
 
+// Several warps may share one 32-point tile (sh_projectors AoS): warp `part` of `SPLIT` evaluates the l-blocks
+// with block_part<SPLIT>(l) == part.  The parts are balanced in work (~l^2 per block) and in columns (2l+1), for two
+// warps {0, 3, 4, 7, 8} | {1, 2, 5, 6, 9}: 49 | 51 columns at lmax = 9.
+template <int SPLIT>
+__host__ __device__ constexpr int block_part(int l) {
+    if (SPLIT == 2) return ((l + 1) >> 1) & 1;
+    if (SPLIT == 4) { constexpr int t[10] = {2, 1, 1, 3, 2, 3, 3, 2, 1, 0}; return t[l % 10]; }   // {9} {8,2,1} {7,4,0} {6,5,3}
+    return 0;
+}
+template <int SPLIT, int PART, int LMAX>
+constexpr int part_mmax() {   // largest m the part's blocks need
+    int m = 0;
+    for (int l = 0; l <= LMAX; ++l)
+        if (block_part<SPLIT>(l) == PART) m = l;
+    return m;
+}
+
 // the real harmonics of block l in ascending m (a3-a5), handed to the sink one block at a time
 // FAST: Horner-in-z^2 polar factors and the azimuthal recurrence instead of the factorized forms -- ~35 % fewer FP64
 // instructions, accuracy still two orders inside the tolerance; sh_project only, on request.
-template <int LMAX, bool FAST = false, class Sink>
+template <int LMAX, bool FAST = false, int SPLIT = 1, int PART = 0, class Sink>
 __device__ __forceinline__ void eval_projector_blocks(const UnitVec& u, const ProjPlan& plan, Sink& sink) {
-    const Azim<LMAX, double, FAST> az(u.x, u.y);
+    constexpr int MMAX = part_mmax<SPLIT, PART, LMAX>();
+    const Azim<MMAX, double, FAST> az(u.x, u.y);
     [[maybe_unused]] const double z2 = u.z * u.z;
     static_for<0, LMAX + 1>([&](auto lc) {
         constexpr int L = decltype(lc)::value;
-        if (plan.first[L] != plan.first[L + 1]) {
-            double blk[2 * L + 1];
-            static_for<0, L + 1>([&](auto mc) {
-                constexpr int M = decltype(mc)::value;
-                constexpr double A = shgen::A_REAL[L][M];
-                double q;
-                if constexpr (FAST) q = A * shgen::PolarHorner<L, M, double>::eval(u.z, z2);
-                else q = A * shgen::Polar<L, M, double>::eval(u.z);
-                if constexpr (M == 0) {
-                    if constexpr (L > 0 && L % 2 == 0) q = zero_where(u.origin, q);   // P_l(0) != 0: the r = 0 convention needs it
-                    blk[L] = q;
-                } else {
-                    blk[L - M] = q * az.S[M];
-                    blk[L + M] = q * az.C[M];
-                }
-            });
-            sink.template block<L>(blk);
+        if constexpr (block_part<SPLIT>(L) == PART) {
+            if (plan.first[L] != plan.first[L + 1]) {
+                double blk[2 * L + 1];
+                static_for<0, L + 1>([&](auto mc) {
+                    constexpr int M = decltype(mc)::value;
+                    constexpr double A = shgen::A_REAL[L][M];
+                    double q;
+                    if constexpr (FAST) q = A * shgen::PolarHorner<L, M, double>::eval(u.z, z2);
+                    else q = A * shgen::Polar<L, M, double>::eval(u.z);
+                    if constexpr (M == 0) {
+                        if constexpr (L > 0 && L % 2 == 0) q = zero_where(u.origin, q);   // P_l(0) != 0: the r = 0 convention needs it
+                        blk[L] = q;
+                    } else {
+                        blk[L - M] = q * az.S[M];
+                        blk[L + M] = q * az.C[M];
+                    }
+                });
+                sink.template block<L>(blk);
+            }
         }
     });
 }
@@ -86,6 +106,7 @@ struct ProjSoASink {
     const ProjPlan& plan;
     const RadialPos& pos;
     template <int L> __device__ __forceinline__ void block(const double (&blk)[2 * L + 1]) {
+#pragma unroll 1   // code size is instruction-fetch traffic (see ProjRowSink)
         for (int s = plan.first[L]; s < plan.first[L + 1]; ++s) {
             const double f = pos.f(radial, plan.nr, plan.chan[s]);
             double* q = p + (int64_t)plan.col[s] * n;
@@ -107,21 +128,29 @@ __global__ void __launch_bounds__(256) sh_proj_soa_kernel(const double* __restri
     eval_projector_blocks<LMAX>(pt.unit(SH_COORDS_CARTESIAN), plan, sink);
 }
 
-// sh_projectors, AoS: one warp = one 32-point tile.  Each lane stages its point's row in the warp's shared-memory tile
-// with 8-byte stores at runtime column offsets; the tile is one contiguous span of `out`.  Copy-out, by `mode`:
+// sh_projectors, AoS: one CTA = one 32-point tile = SPLIT warps; lane i of every warp takes point i of the tile, and warp w
+// evaluates the l-blocks of part w (block_part): a2/a3 are repeated per warp, but a tile's chain of dependent FP64
+// instructions is cut SPLIT-fold.  That chain, not the store, is what bounds this kernel: shared memory caps an SM at
+// eight 25.6 KB tiles (100 columns), and with one warp per tile that is two warps per scheduler running ~2200
+// instructions per tile at one issue every ~6 cycles.  Each lane stages its point's columns in the tile with 8-byte
+// stores at runtime column offsets; the tile is one contiguous span of `out`.  Copy-out, by `mode`:
 //   PROJ_AOS_TILEBULK (`out` 16-byte aligned, ncols not a multiple of 8): rows staged densely (pitch = ncols; the 8-byte
 //       staging stores conflict gcd(ncols, 16)-way, i.e. not at all for odd ncols), one TMA bulk copy
-//       (cp.async.bulk.global.shared::cta) of the whole tile by lane 0; one warp per CTA (see TILEBULK_WARPS);
+//       (cp.async.bulk.global.shared::cta) of the whole tile by thread 0; one tile per CTA, so the CTA-scoped
+//       fence.proxy.async never waits for another tile's copy;
 //   PROJ_AOS_ROWBULK (ncols a multiple of 8, `out` 16-byte aligned): pitch = ncols + 2 (rows stay 16-byte aligned, staging
-//       stores conflict 2-way), one bulk copy per row by its lane (32 copies issued one after the other);
-//   PROJ_AOS_PLAIN: pitch odd, the warp copies the tile out with coalesced streaming stores (any alignment, any width).
-// A ragged last tile is always copied out by the warp.
+//       stores conflict 2-way), one bulk copy per row by the lanes of warp 0 (32 copies issued one after the other);
+//   PROJ_AOS_PLAIN: pitch odd, the CTA copies the tile out with coalesced streaming stores (any alignment, any width).
+// A ragged last tile is always copied out by the CTA; its idle lanes evaluate the last point.
 constexpr int PROJ_AOS_PLAIN = 0, PROJ_AOS_ROWBULK = 1, PROJ_AOS_TILEBULK = 2;
 struct ProjRowSink {
     double* row;
     const double* fs;   // this lane's radial values: fs[slot*32]
     const ProjPlan& plan;
     template <int L> __device__ __forceinline__ void block(const double (&blk)[2 * L + 1]) {
+        // not unrolled: the kernel is straight-line code that every warp runs through once per tile, so its size is
+        // instruction-fetch traffic (4096 -> ~2300 SASS instructions at lmax = 9)
+#pragma unroll 1
         for (int s = plan.first[L]; s < plan.first[L + 1]; ++s) {
             const double f = fs[s * 32];
             double* q = row + plan.col[s];
@@ -130,34 +159,42 @@ struct ProjRowSink {
     }
 };
 
-template <int LMAX>
-__global__ void __launch_bounds__(128) sh_proj_aos_kernel(const double* __restrict__ xyz, int64_t n, const double* __restrict__ radial,
-                                                           const __grid_constant__ ProjPlan plan, double* __restrict__ out, int pitch, int mode,
-                                                           InputPrefetch pf) {
+template <int LMAX, int SPLIT>
+__global__ void __launch_bounds__(32 * SPLIT) sh_proj_aos_kernel(const double* __restrict__ xyz, int64_t n, const double* __restrict__ radial,
+                                                                  const __grid_constant__ ProjPlan plan, double* __restrict__ out, int pitch, int mode,
+                                                                  InputPrefetch pf) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, warps = blockDim.x >> 5;
-    prefetch_input_window(xyz, n * 24, (int64_t)warps * 32 * 24, pf);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    prefetch_input_window(xyz, n * 24, (int64_t)32 * 24, pf);
     const int ncols = plan.ncols;
     const int nslots = plan.first[shgen::LMAX_CAP + 1];
-    double* tile = reinterpret_cast<double*>(smem_raw) + (size_t)warp * 32 * (pitch + nslots);
+    double* tile = reinterpret_cast<double*>(smem_raw);
     double* fs = tile + 32 * pitch;   // radial values [slot][lane]
-    const int64_t base = ((int64_t)blockIdx.x * warps + warp) << 5;
-    if (base >= n) return;
-    const int64_t i = base + lane;
+    const int64_t base = (int64_t)blockIdx.x << 5;
     const int rows = (n - base) < 32 ? (int)(n - base) : 32;
-    if (i < n) {
-        RawPoint<double> pt;
-        pt.load(xyz, i);
-        const RadialPos pos(pt.x, pt.y, pt.z, plan);
-        stage_radial(pos, radial, plan, fs, lane, 1.0);
-        ProjRowSink sink{tile + lane * pitch, fs + lane, plan};
-        eval_projector_blocks<LMAX>(pt.unit(SH_COORDS_CARTESIAN), plan, sink);
-    }
+    const int64_t i = lane < rows ? base + lane : n - 1;
+    RawPoint<double> pt;
+    pt.load(xyz, i);
+    const RadialPos pos(pt.x, pt.y, pt.z, plan);
+    // radial values of every channel slot at this lane's point: the warps share the slots (independent table loads overlap)
+#pragma unroll 4
+    for (int s = warp; s < nslots; s += SPLIT) fs[s * 32 + lane] = pos.f(radial, plan.nr, plan.chan[s]);
+    if constexpr (SPLIT > 1) __syncthreads();
+    else __syncwarp();
+    const UnitVec u = pt.unit(SH_COORDS_CARTESIAN);
+    ProjRowSink sink{tile + lane * pitch, fs + lane, plan};
+    static_for<0, SPLIT>([&](auto pc) {
+        constexpr int PART = decltype(pc)::value;
+        if (warp == PART) eval_projector_blocks<LMAX, false, SPLIT, PART>(u, plan, sink);
+    });
     double* g = out + base * ncols;
-    if (mode != PROJ_AOS_PLAIN && rows == 32) {
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // every lane: its staging stores -> async proxy
+    const bool bulk = mode != PROJ_AOS_PLAIN && rows == 32;
+    if (bulk) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // every thread: its staging stores -> async proxy
+    if constexpr (SPLIT > 1) __syncthreads();
+    else __syncwarp();
+    if (bulk) {
+        if (warp != 0) return;
         if (mode == PROJ_AOS_TILEBULK) {
-            __syncwarp();
             if (lane == 0)
                 asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(g), "r"(smem_u32(tile)), "r"(32 * ncols * 8) : "memory");
         } else {
@@ -169,13 +206,12 @@ __global__ void __launch_bounds__(128) sh_proj_aos_kernel(const double* __restri
         asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory is released when the CTA exits
         return;
     }
-    __syncwarp();
     const int total = rows * ncols;
-    int r = 0, c = lane;
+    int r = 0, c = threadIdx.x;
     while (c >= ncols) { c -= ncols; ++r; }
-    for (int e = lane; e < total; e += 32) {
+    for (int e = threadIdx.x; e < total; e += 32 * SPLIT) {
         __stcs(g + e, tile[r * pitch + c]);
-        c += 32;
+        c += 32 * SPLIT;
         while (c >= ncols) { c -= ncols; ++r; }
     }
 }
@@ -257,6 +293,7 @@ struct ProjectSink {
     }
 
     template <int L> __device__ __forceinline__ void block(const double (&blk)[2 * L + 1]) {
+#pragma unroll 1   // code size is instruction-fetch traffic (see ProjRowSink)
         for (int s = plan.first[L]; s < plan.first[L + 1]; ++s) {
             const double f = fs[s * 32];
             const int c0 = seg.scol[s], b0 = seg.sbeg[s];
@@ -407,12 +444,32 @@ int check_projector_args(const double* xyz, int64_t n, int nproj, const int* pro
 
 constexpr int PROJ_CTAS_PER_SM = PROJ_CTAS_NV1 > PROJ_CTAS_NV4 ? PROJ_CTAS_NV1 : PROJ_CTAS_NV4;   // grid cap of sh_project_kernel: the machine filled once (what the workspace is sized for)
 
+// warps per tile (block_part): the default comes from the 128^3-grid measurements in DESIGN.md section 6
+#ifndef SHB200_PROJ_AOS_SPLIT
+#define SHB200_PROJ_AOS_SPLIT 2
+#endif
+
+template <int LMAX, int SPLIT>
+int launch_proj_aos_split(const double* xyz, int64_t n, const double* radial, const ProjPlan& plan, double* out, int pitch, int mode, size_t smem,
+                          cudaStream_t st) {
+    auto kern = sh_proj_aos_kernel<LMAX, SPLIT>;
+    static size_t smem_set = 0;   // the opt-in limit only ever grows
+    if (smem > 48 * 1024 && smem > smem_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return cuda_fail(e);
+        smem_set = smem;
+    }
+    const int64_t ntiles = (n + 31) / 32;
+    if (ntiles > 0x7fffffffLL) return SH_ERR_COUNT;
+    kern<<<(unsigned)ntiles, 32 * SPLIT, smem, st>>>(xyz, n, radial, plan, out, pitch, mode, prefetch_plan(n, 32));
+    return launch_status();
+}
+
 template <int LMAX>
 int launch_proj_aos(const double* xyz, int64_t n, const double* radial, const ProjPlan& plan, double* out, cudaStream_t st) {
-    auto kern = sh_proj_aos_kernel<LMAX>;
     const int ncols = plan.ncols;
     // store mode (see the kernel): bulk copies need a 16-byte aligned `out` and a tile that leaves room for >= 4 CTAs per SM
-    int mode = PROJ_AOS_PLAIN, pitch = ncols | 1, warps = 4;
+    int mode = PROJ_AOS_PLAIN, pitch = ncols | 1;
     if (aligned(out, 16) && (size_t)32 * (ncols + 2 + plan.first[shgen::LMAX_CAP + 1]) * sizeof(double) <= (size_t)55 * 1024) {
         // dense rows conflict gcd(ncols, 16)-way on the 8-byte staging stores (16 lanes per wavefront, rows ncols words apart)
         int g = 16;
@@ -424,23 +481,17 @@ int launch_proj_aos(const double* xyz, int64_t n, const double* radial, const Pr
         else if (force == 3) mode = PROJ_AOS_TILEBULK;
         if (mode == PROJ_AOS_TILEBULK) pitch = ncols;
         else if (mode == PROJ_AOS_ROWBULK) pitch = (ncols / 2) & 1 ? ncols : ncols + 2;
-        if (mode != PROJ_AOS_PLAIN) warps = TILEBULK_WARPS;   // fence.proxy.async is CTA-scoped: one warp per CTA keeps the warps' copies independent
     }
-    const size_t per_warp = (size_t)32 * (pitch + plan.first[shgen::LMAX_CAP + 1]) * sizeof(double);   // row tile + radial values
-    while (warps > 1 && warps * per_warp > (size_t)56 * 1024) warps >>= 1;   // four CTAs per SM while the row width allows it
-    const size_t smem = warps * per_warp;
+    const size_t smem = (size_t)32 * (pitch + plan.first[shgen::LMAX_CAP + 1]) * sizeof(double);   // row tile + radial values
     if (smem > (size_t)227 * 1024) return SH_ERR_PROJECTOR;
-    static size_t smem_set = 0;   // the opt-in limit only ever grows
-    if (smem > 48 * 1024 && smem > smem_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return cuda_fail(e);
-        smem_set = smem;
+    // warps per tile: splitting pays once there are several l-blocks to share
+    int split = LMAX >= 4 ? tuned(SH_TUNE_PROJ_AOS_SPLIT, SHB200_PROJ_AOS_SPLIT) : 1;
+    if constexpr (LMAX >= 4) {
+        if (split >= 4) return launch_proj_aos_split<LMAX, 4>(xyz, n, radial, plan, out, pitch, mode, smem, st);
+        if (split >= 2) return launch_proj_aos_split<LMAX, 2>(xyz, n, radial, plan, out, pitch, mode, smem, st);
     }
-    const int64_t ntiles = (n + 31) / 32;
-    const int64_t blocks = (ntiles + warps - 1) / warps;
-    if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
-    kern<<<(unsigned)blocks, warps * 32, smem, st>>>(xyz, n, radial, plan, out, pitch, mode, prefetch_plan(n, (int64_t)warps * 32));
-    return launch_status();
+    (void)split;
+    return launch_proj_aos_split<LMAX, 1>(xyz, n, radial, plan, out, pitch, mode, smem, st);
 }
 
 template <int LMAX>

@@ -137,8 +137,11 @@ __global__ void __launch_bounds__(256) sh_soa_pair_kernel(const float* __restric
         if (have_next) load6(j + 256, na, nb, nc);
         if (have) {
             SoAPairSink sink{out + 2 * j, n};
-            if (coords == SH_COORDS_CARTESIAN) evaluate_pair<LMAX>(normalize(ca.x, ca.y, cb.x), normalize(cb.y, cc.x, cc.y), sink);
-            else evaluate_pair<LMAX>(as_given(ca.x, ca.y, cb.x), as_given(cb.y, cc.x, cc.y), sink);
+            // one copy of the polynomial code: only the front end branches (straight-line code size is instruction-fetch traffic)
+            UnitVec u0, u1;
+            if (coords == SH_COORDS_CARTESIAN) { u0 = normalize(ca.x, ca.y, cb.x); u1 = normalize(cb.y, cc.x, cc.y); }
+            else { u0 = as_given(ca.x, ca.y, cb.x); u1 = as_given(cb.y, cc.x, cc.y); }
+            evaluate_pair<LMAX>(u0, u1, sink);
         }
         ca = na; cb = nb; cc = nc;
         have = have_next;

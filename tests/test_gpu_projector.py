@@ -115,11 +115,12 @@ def test_every_lmax_unsorted_channels_and_ragged_sizes(sh, oracle_mod, lmax):
         check_project(gpu_project(sh, pts, proj_l, tab, dr, w), coeff, abs_sum)
 
 
-@pytest.mark.parametrize("proj_l", [[2], [0, 1, 3], [1, 1], [0, 2, 1, 3], [9, 9, 9, 4, 0], [9] * 11, [9] * 12])
+@pytest.mark.parametrize("proj_l", [[2], [0, 1, 3], [1, 1], [0, 2, 1, 3], [9, 9, 9, 4, 0], [0, 1, 2, 3, 4, 5, 6, 7, 8, 9], [5, 4, 4, 7], [9] * 11, [9] * 12])
 def test_aos_store_modes(sh, oracle_mod, proj_l):
     """AoS copy-out modes of sh_projectors: odd ncols (one bulk copy per tile), even ncols with ncols/2 odd or even (one
     bulk copy per row, padded pitch), rows too wide for the bulk tile (12 x 19 = 228 columns), a misaligned `out` (warp copy);
-    full tiles, a ragged tail and fewer points than one tile."""
+    full tiles, a ragged tail and fewer points than one tile; one, two or four warps per tile (each evaluating part of the
+    l-blocks)."""
     rng = np.random.default_rng(len(proj_l) * 31 + proj_l[0])
     nr, dr = 33, 0.1
     tab = rng.standard_normal((len(proj_l), nr))
@@ -130,12 +131,15 @@ def test_aos_store_modes(sh, oracle_mod, proj_l):
         want = oracle_mod.projectors(pts, proj_l, tab, dr)
         for mis in (0, 1, 2):
             for mode in (0, 1, 2, 3):   # automatic, then each copy-out forced (where it applies)
-                sh.set_tuning("proj_aos_mode", mode)
-                try:
-                    got = gpu_projectors(sh, pts, proj_l, tab, dr, "aos", misalign=mis)
-                finally:
-                    sh.set_tuning("proj_aos_mode", 0)
-                assert np.abs(got - want).max() <= TOL * max(1.0, np.abs(tab).max()), (n, mis, mode)
+                for split in (0, 1, 2, 4):   # warps sharing a tile (lmax >= 4): default, then each forced
+                    sh.set_tuning("proj_aos_mode", mode)
+                    sh.set_tuning("proj_aos_split", split)
+                    try:
+                        got = gpu_projectors(sh, pts, proj_l, tab, dr, "aos", misalign=mis)
+                    finally:
+                        sh.set_tuning("proj_aos_mode", 0)
+                        sh.set_tuning("proj_aos_split", 0)
+                    assert np.abs(got - want).max() <= TOL * max(1.0, np.abs(tab).max()), (n, mis, mode, split)
 
 
 @pytest.mark.parametrize("form", [0, 1])
