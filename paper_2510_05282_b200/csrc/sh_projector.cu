@@ -250,6 +250,44 @@ struct ProjSegments {
     unsigned char flush[SH_MAX_PROJ];   // slot -> 1 if the segment is complete after this slot
 };
 
+// column sums of a complete segment, added to the warp's running sums
+template <int NV>
+__device__ __forceinline__ void project_flush(double* tile, double* sums, const double* wt, int lane, int begin, int len) {
+    __syncwarp();
+    if (lane < len) {
+        const double2* t = reinterpret_cast<const double2*>(tile + lane * PROJ_SEG_PITCH);
+        if constexpr (NV == 1) {
+            double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+#pragma unroll
+            for (int r = 0; r < 16; r += 2) {
+                const double2 a = t[r], b = t[r + 1];
+                s0 += a.x; s1 += a.y; s2 += b.x; s3 += b.y;
+            }
+            sums[begin + lane] += (s0 + s1) + (s2 + s3);
+        } else {
+            const double2* wv = reinterpret_cast<const double2*>(wt);   // row r: (w0, w1), (w2, w3)
+            double e[PROJ_NV], o[PROJ_NV];
+            static_for<0, PROJ_NV>([&](auto vc) { e[decltype(vc)::value] = 0.0; o[decltype(vc)::value] = 0.0; });
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                const double2 a = t[r];   // points 2r, 2r+1
+                const double2 w01 = wv[4 * r], w23 = wv[4 * r + 1], x01 = wv[4 * r + 2], x23 = wv[4 * r + 3];
+                e[0] = fma(a.x, w01.x, e[0]); e[1] = fma(a.x, w01.y, e[1]); e[2] = fma(a.x, w23.x, e[2]); e[3] = fma(a.x, w23.y, e[3]);
+                o[0] = fma(a.y, x01.x, o[0]); o[1] = fma(a.y, x01.y, o[1]); o[2] = fma(a.y, x23.x, o[2]); o[3] = fma(a.y, x23.y, o[3]);
+            }
+            static_for<0, PROJ_NV>([&](auto vc) {
+                constexpr int V = decltype(vc)::value;
+                sums[V * PROJ_MAX_COLS + begin + lane] += e[V] + o[V];
+            });
+        }
+    }
+    __syncwarp();
+}
+
+__device__ __noinline__ void project_flush_call(double* tile, double* sums, const double* wt, int lane, int begin, int len) {
+    project_flush<PROJ_NV>(tile, sums, wt, lane, begin, len);
+}
+
 template <int NV>
 struct ProjectSink {
     double* tile;        // the warp's [32][PROJ_SEG_PITCH] transposed segment tile
@@ -260,36 +298,12 @@ struct ProjectSink {
     const ProjSegments& seg;
     int lane;
 
+    // NV = 4: out of line.  Inlined after every l-block its 210 instructions stand ten times in code that a warp runs through
+    // once per tile (4744 -> 2552 SASS instructions at lmax 9; 0.334 -> 0.327 ms on the 128^3 grid).  The 36 instructions of
+    // NV = 1 stay inline (the call costs more than the fetches: 0.189 -> 0.202 ms out of line).
     __device__ __forceinline__ void flush(int begin, int len) {
-        __syncwarp();
-        if (lane < len) {
-            const double2* t = reinterpret_cast<const double2*>(tile + lane * PROJ_SEG_PITCH);
-            if constexpr (NV == 1) {
-                double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
-#pragma unroll
-                for (int r = 0; r < 16; r += 2) {
-                    const double2 a = t[r], b = t[r + 1];
-                    s0 += a.x; s1 += a.y; s2 += b.x; s3 += b.y;
-                }
-                sums[begin + lane] += (s0 + s1) + (s2 + s3);
-            } else {
-                const double2* wv = reinterpret_cast<const double2*>(wt);   // row r: (w0, w1), (w2, w3)
-                double e[PROJ_NV], o[PROJ_NV];
-                static_for<0, PROJ_NV>([&](auto vc) { e[decltype(vc)::value] = 0.0; o[decltype(vc)::value] = 0.0; });
-#pragma unroll
-                for (int r = 0; r < 16; ++r) {
-                    const double2 a = t[r];   // points 2r, 2r+1
-                    const double2 w01 = wv[4 * r], w23 = wv[4 * r + 1], x01 = wv[4 * r + 2], x23 = wv[4 * r + 3];
-                    e[0] = fma(a.x, w01.x, e[0]); e[1] = fma(a.x, w01.y, e[1]); e[2] = fma(a.x, w23.x, e[2]); e[3] = fma(a.x, w23.y, e[3]);
-                    o[0] = fma(a.y, x01.x, o[0]); o[1] = fma(a.y, x01.y, o[1]); o[2] = fma(a.y, x23.x, o[2]); o[3] = fma(a.y, x23.y, o[3]);
-                }
-                static_for<0, PROJ_NV>([&](auto vc) {
-                    constexpr int V = decltype(vc)::value;
-                    sums[V * PROJ_MAX_COLS + begin + lane] += e[V] + o[V];
-                });
-            }
-        }
-        __syncwarp();
+        if constexpr (NV == 1) project_flush<1>(tile, sums, wt, lane, begin, len);
+        else project_flush_call(tile, sums, wt, lane, begin, len);
     }
 
     template <int L> __device__ __forceinline__ void block(const double (&blk)[2 * L + 1]) {
