@@ -377,6 +377,9 @@ def run_ours(args):
 
     _build.ensure_built()  # compiles only if the in-tree library is absent
     sh.load()  # no fallback: fails here if libshb200.so cannot be loaded
+    tune = {k: int(v) for k, v in (t.split("=", 1) for t in args.tune)}
+    for knob, value in tune.items():
+        sh.set_tuning(knob, value)
     rank, local, world = env_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the CUDA path has no CPU fallback)")
@@ -473,7 +476,8 @@ def run_ours(args):
             "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": WORKLOAD, "points_per_gpu": n, "lmax": LMAX, "calls_per_step": ["sh_real SOA", "sh_real AOS"],
-                       "l2": "outputs (1.68 GB per call) and rotating input replicas (4 x 50 MB) exceed the 126 MB L2"},
+                       "l2": "outputs (1.68 GB per call) and rotating input replicas (4 x 50 MB) exceed the 126 MB L2",
+                       **({"tune": tune} if tune else {})},
             "gpu_launches": int(launches),
             "clocks": clocks,
             "kernels": {
@@ -508,6 +512,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the untimed-by-`value` runs of the other configs")
+    ap.add_argument("--tune", action="append", default=[], metavar="KNOB=VALUE",
+                    help="override a launch heuristic for the whole run (binding.TUNE names, e.g. soa_split=2); recorded in config")
     ap.add_argument("--only", default=None, help="run only the other-config cases whose name contains this substring")
     args = ap.parse_args()
     if args.impl == "reference":

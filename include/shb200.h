@@ -173,7 +173,8 @@ enum {
     SH_TUNE_PROJECT_FORM = 5,       /* sh_project polynomials: 0 = the factorized forms of every other call (default); 1 = Horner in z^2 for the
                                        polar factors and (x + iy)^m by recurrence: ~35 % fewer FP64 instructions, same tolerance */
     SH_TUNE_PROJ_AOS_SPLIT = 6,     /* sh_projectors AoS, lmax >= 4: warps that share one 32-point tile, each evaluating part of the l-blocks: 1, 2 (default) or 4 */
-    SH_TUNE_COUNT = 7
+    SH_TUNE_SOA_SPLIT = 7,          /* sh_real SoA tensor-store path, lmax >= 4: warps that share a 32-point group of the tile, each evaluating part of the l-blocks: 1 or 2 (default) */
+    SH_TUNE_COUNT = 8
 };
 int sh_set_tuning(int knob, int value);
 

@@ -110,7 +110,7 @@ def index_spinor(l: int, twoj: int, twomj: int) -> int:
     return load().sh_index_spinor(l, twoj, twomj)
 
 
-TUNE = {"soa_tiles_per_cta": 0, "aos_tiles_per_warp": 1, "prefetch_window_points": 2, "proj_aos_mode": 3, "soa_tma": 4, "project_form": 5, "proj_aos_split": 6}
+TUNE = {"soa_tiles_per_cta": 0, "aos_tiles_per_warp": 1, "prefetch_window_points": 2, "proj_aos_mode": 3, "soa_tma": 4, "project_form": 5, "proj_aos_split": 6, "soa_split": 7}
 
 
 def set_tuning(knob, value: int) -> None:

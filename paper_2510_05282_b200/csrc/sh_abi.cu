@@ -26,7 +26,7 @@ int sm_count() {
 }
 
 // launch-heuristic overrides (sh_set_tuning); 0 = default
-std::atomic<int> g_tune[8];
+std::atomic<int> g_tune[SH_TUNE_COUNT];
 
 int tuned(int knob, int dflt) {
     const int v = g_tune[knob].load(std::memory_order_relaxed);

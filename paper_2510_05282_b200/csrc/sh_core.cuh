@@ -203,36 +203,67 @@ struct Azim {
     }
 };
 
+// block l of the real harmonics, m = -l..l, from the azimuthal factors (MAZ >= L of them)
+template <int L, int MAZ, typename T, class O, class Sink>
+__device__ __forceinline__ void real_block(const Azim<MAZ, T>& az, T z, O origin, Sink& sink) {
+    static_assert(MAZ >= L, "azimuthal factors up to m = l");
+    T q[L + 1];
+    static_for<0, L + 1>([&](auto mc) {
+        constexpr int M = decltype(mc)::value;
+        constexpr double A = shgen::A_REAL[L][M];
+        q[M] = T(A) * shgen::Polar<L, M, T>::eval(z);
+    });
+    // r = 0: x = y = z = 0 zeroes everything except the even-l, m = 0 polynomials (P_l(0) != 0)
+    if constexpr (L > 0 && L % 2 == 0) q[0] = zero_where(origin, q[0]);
+    sink.template polar<L>(q);   // the normalized polar factors of block l (seeds of the l > 9 recurrence)
+    static_for<0, L>([&](auto jc) {
+        constexpr int M = L - decltype(jc)::value;
+        sink.template put1<L * (L + 1) - M>(q[M] * az.S[M]);
+    });
+    sink.template put1<L * (L + 1)>(q[0]);
+    static_for<1, L + 1>([&](auto mc) {
+        constexpr int M = decltype(mc)::value;
+        sink.template put1<L * (L + 1) + M>(q[M] * az.C[M]);
+    });
+    sink.template end_l<L>();
+}
+
 template <int LMAX, typename T, class O, class Sink>
 __device__ __forceinline__ void eval_real(const Azim<LMAX, T>& az, T z, O origin, Sink& sink) {
-    static_for<0, LMAX + 1>([&](auto lc) {
-        constexpr int L = decltype(lc)::value;
-        T q[L + 1];
-        static_for<0, L + 1>([&](auto mc) {
-            constexpr int M = decltype(mc)::value;
-            constexpr double A = shgen::A_REAL[L][M];
-            q[M] = T(A) * shgen::Polar<L, M, T>::eval(z);
-        });
-        // r = 0: x = y = z = 0 zeroes everything except the even-l, m = 0 polynomials (P_l(0) != 0)
-        if constexpr (L > 0 && L % 2 == 0) q[0] = zero_where(origin, q[0]);
-        sink.template polar<L>(q);   // the normalized polar factors of block l (seeds of the l > 9 recurrence)
-        static_for<0, L>([&](auto jc) {
-            constexpr int M = L - decltype(jc)::value;
-            sink.template put1<L * (L + 1) - M>(q[M] * az.S[M]);
-        });
-        sink.template put1<L * (L + 1)>(q[0]);
-        static_for<1, L + 1>([&](auto mc) {
-            constexpr int M = decltype(mc)::value;
-            sink.template put1<L * (L + 1) + M>(q[M] * az.C[M]);
-        });
-        sink.template end_l<L>();
-    });
+    static_for<0, LMAX + 1>([&](auto lc) { real_block<decltype(lc)::value>(az, z, origin, sink); });
 }
 
 template <int LMAX, typename T, class O, class Sink>
 __device__ __forceinline__ void eval_real(T x, T y, T z, O origin, Sink& sink) {
     const Azim<LMAX, T> az(x, y);
     eval_real<LMAX, T>(az, z, origin, sink);
+}
+
+// Several warps may share the points of one tile, warp `PART` of `SPLIT` evaluating the l-blocks with
+// block_part<SPLIT>(l) == PART: a2/a3 are repeated per warp, the chain of dependent instructions per tile is cut SPLIT-fold.
+// The parts are balanced in work (~l^2 per block) and in values (2l+1): for two warps {0, 3, 4, 7, 8} | {1, 2, 5, 6, 9},
+// 49 | 51 values at lmax = 9.
+template <int SPLIT>
+__host__ __device__ constexpr int block_part(int l) {
+    if (SPLIT == 2) return ((l + 1) >> 1) & 1;
+    if (SPLIT == 4) { constexpr int t[10] = {2, 1, 1, 3, 2, 3, 3, 2, 1, 0}; return t[l % 10]; }   // {9} {8,2,1} {7,4,0} {6,5,3}
+    return 0;
+}
+template <int SPLIT, int PART, int LMAX>
+constexpr int part_mmax() {   // largest m the part's blocks need
+    int m = 0;
+    for (int l = 0; l <= LMAX; ++l)
+        if (block_part<SPLIT>(l) == PART) m = l;
+    return m;
+}
+
+template <int LMAX, int SPLIT, int PART, class O, class Sink>
+__device__ __forceinline__ void eval_real_part(double x, double y, double z, O origin, Sink& sink) {
+    const Azim<part_mmax<SPLIT, PART, LMAX>(), double> az(x, y);
+    static_for<0, LMAX + 1>([&](auto lc) {
+        constexpr int L = decltype(lc)::value;
+        if constexpr (block_part<SPLIT>(L) == PART) real_block<L>(az, z, origin, sink);
+    });
 }
 
 // a[M] + i b[M] = B_lm Qhat_lm (C_M + i S_M);  Y_l^{-M} = (a, -b),  Y_l^{+M} = (-1)^M (a, b)

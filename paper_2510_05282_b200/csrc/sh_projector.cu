@@ -49,23 +49,6 @@ __device__ __forceinline__ void stage_radial(const RadialPos& pos, const double*
     for (int s = 0; s < nslots; ++s) fs[s * 32 + lane] = pos.f(radial, plan.nr, plan.chan[s]) * scale;
 }
 
-// Several warps may share one 32-point tile (sh_projectors AoS): warp `part` of `SPLIT` evaluates the l-blocks
-// with block_part<SPLIT>(l) == part.  The parts are balanced in work (~l^2 per block) and in columns (2l+1), for two
-// warps {0, 3, 4, 7, 8} | {1, 2, 5, 6, 9}: 49 | 51 columns at lmax = 9.
-template <int SPLIT>
-__host__ __device__ constexpr int block_part(int l) {
-    if (SPLIT == 2) return ((l + 1) >> 1) & 1;
-    if (SPLIT == 4) { constexpr int t[10] = {2, 1, 1, 3, 2, 3, 3, 2, 1, 0}; return t[l % 10]; }   // {9} {8,2,1} {7,4,0} {6,5,3}
-    return 0;
-}
-template <int SPLIT, int PART, int LMAX>
-constexpr int part_mmax() {   // largest m the part's blocks need
-    int m = 0;
-    for (int l = 0; l <= LMAX; ++l)
-        if (block_part<SPLIT>(l) == PART) m = l;
-    return m;
-}
-
 // the real harmonics of block l in ascending m (a3-a5), handed to the sink one block at a time
 // FAST: Horner-in-z^2 polar factors and the azimuthal recurrence instead of the factorized forms -- ~35 % fewer FP64
 // instructions, accuracy still two orders inside the tolerance; sh_project only, on request.

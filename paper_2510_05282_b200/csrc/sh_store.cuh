@@ -72,6 +72,12 @@ __global__ void __launch_bounds__(256) sh_soa_kernel(const TI* __restrict__ xyz,
 // (rows of 256 B .. 2 KB; 8 warps = one 205 KB tile per SM, nothing overlaps) on the 128^3 grid at lmax = 9.
 // (The fp32 variant gains nothing from it -- 255 vs 257 us on 2^22 points -- and stays on sh_soa_pair_kernel.)
 constexpr int SOA_TMA_WARPS = SHB200_SOA_TMA_WARPS;
+// warps sharing a 32-point group (lmax >= 4): 1 or 2.  Two warps, each evaluating part of the l-blocks, shorten a tile's
+// compute phase, so the two resident CTAs overlap their tensor stores better: 0.2499 -> 0.2477 ms on the 128^3 grid at
+// lmax = 9 (with 64-point tiles the split changes nothing: 0.2585 ms either way -- row length, not compute, bounds those)
+#ifndef SHB200_SOA_SPLIT
+#define SHB200_SOA_SPLIT 2
+#endif
 
 template <int PTS>
 struct TileSink {
@@ -81,22 +87,32 @@ struct TileSink {
     template <int L> __device__ __forceinline__ void polar(const double (&)[L + 1]) {}
 };
 
-template <int LMAX, int WARPS>
-__global__ void __launch_bounds__(32 * WARPS) sh_soa_tma_kernel(const double* __restrict__ xyz, int64_t n, const __grid_constant__ CUtensorMap tmap, int coords,
-                                                                 InputPrefetch pf) {
+// SPLIT warps share each 32-point group of the tile, each evaluating part of the l-blocks (block_part in sh_core.cuh)
+template <int LMAX, int WARPS, int SPLIT>
+__global__ void __launch_bounds__(32 * WARPS * SPLIT) sh_soa_tma_kernel(const double* __restrict__ xyz, int64_t n, const __grid_constant__ CUtensorMap tmap,
+                                                                         int coords, InputPrefetch pf) {
     constexpr int PTS = 32 * WARPS;
     extern __shared__ __align__(128) unsigned char smem_tile[];
     prefetch_input_window(xyz, n * 24, (int64_t)PTS * 24, pf);
     double* tile = reinterpret_cast<double*>(smem_tile);
-    const int64_t base = (int64_t)blockIdx.x * PTS, i = base + threadIdx.x;
+    const int p = SPLIT == 1 ? threadIdx.x : threadIdx.x % PTS;   // point of the tile
+    const int64_t base = (int64_t)blockIdx.x * PTS, i = base + p;
     if (i < n) {
         RawPoint<double> pt;
         pt.load(xyz, i);
-        TileSink<PTS> sink{tile + threadIdx.x};
-        evaluate<KIND_REAL, LMAX, double>(pt.unit(coords), sink);
+        TileSink<PTS> sink{tile + p};
+        const UnitVec u = pt.unit(coords);
+        if constexpr (SPLIT == 1) evaluate<KIND_REAL, LMAX, double>(u, sink);
+        else {
+            const int part = threadIdx.x / PTS;   // warp-uniform
+            static_for<0, SPLIT>([&](auto pc) {
+                constexpr int PART = decltype(pc)::value;
+                if (part == PART) eval_real_part<LMAX, SPLIT, PART>(u.x, u.y, u.z, u.origin, sink);
+            });
+        }
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // every thread: its staging stores -> async proxy
-    if constexpr (WARPS == 1) __syncwarp();
+    if constexpr (WARPS * SPLIT == 1) __syncwarp();
     else __syncthreads();
     if (threadIdx.x == 0) {
         asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];" ::"l"(&tmap), "r"((int)base), "r"(0),
@@ -400,17 +416,20 @@ int launch_soa_tma(const double* xyz, int64_t n, double* out, int coords, cudaSt
     const int64_t blocks = (n + PTS - 1) / PTS;
     constexpr size_t smem = (size_t)K * PTS * sizeof(double);
     static_assert(smem <= 227 * 1024, "tile exceeds shared memory");
-    auto kern = sh_soa_tma_kernel<LMAX, SOA_TMA_WARPS>;
-    if constexpr (smem > 48 * 1024) {
-        static bool opted_in = false;
-        if (!opted_in) {
+    auto launch = [&](auto kern, int split, bool& opted_in) -> int {
+        if (smem > 48 * 1024 && !opted_in) {
             cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e != cudaSuccess) return cuda_fail(e);
             opted_in = true;
         }
+        kern<<<(unsigned)blocks, PTS * split, smem, st>>>(xyz, n, tmap, coords, prefetch_plan(n, PTS));
+        return launch_status();
+    };
+    static bool opted_in[2] = {false, false};
+    if constexpr (LMAX >= 4) {
+        if (tuned(SH_TUNE_SOA_SPLIT, SHB200_SOA_SPLIT) >= 2) return launch(sh_soa_tma_kernel<LMAX, SOA_TMA_WARPS, 2>, 2, opted_in[1]);
     }
-    kern<<<(unsigned)blocks, PTS, smem, st>>>(xyz, n, tmap, coords, prefetch_plan(n, PTS));
-    return launch_status();
+    return launch(sh_soa_tma_kernel<LMAX, SOA_TMA_WARPS, 1>, 1, opted_in[0]);
 }
 
 // staging capacity per row, in scalars: whole rows for real (800 B at lmax = 9) and complex (1600 B);

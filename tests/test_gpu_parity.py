@@ -131,6 +131,13 @@ def test_soa_tensor_store_and_lsu_store_paths(sh, oracle_mod, lmax):
             sh.set_tuning("soa_tma", 0)
         assert max_err(got_tma, want) <= TOL64 and max_err(got_lsu, want) <= TOL64, n
         assert np.array_equal(got_tma, got_lsu), n
+        for split in (1, 2):   # one warp per 32-point group, or two sharing it (each evaluating part of the l-blocks)
+            sh.set_tuning("soa_split", split)
+            try:
+                got = gpu_eval(sh, "real", pts, lmax, "soa")
+            finally:
+                sh.set_tuning("soa_split", 0)
+            assert np.array_equal(got, got_lsu), (n, split)
 
 
 @pytest.mark.parametrize("kind", ["real", "complex", "spinor"])
