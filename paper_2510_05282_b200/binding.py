@@ -6,6 +6,7 @@ There is no CPU fallback: if the shared library is missing or a call fails, an e
 from __future__ import annotations
 
 import ctypes
+import math
 import os
 
 import numpy as np
@@ -149,11 +150,15 @@ def _device_call(kind: str, xyz, lmax: int, out, layout, store, stream, coords="
     shape = out_shape(kind, n, lmax, layout)
     if out is None:
         out = torch.empty(shape, dtype=want, device=xyz.device)
-    elif not (out.is_cuda and out.dtype == want and out.is_contiguous() and out.numel() == int(np.prod(shape))):
-        raise ValueError(f"out must be a contiguous CUDA tensor of {want} with {int(np.prod(shape))} elements")
+    elif not (out.is_cuda and out.dtype == want and out.is_contiguous() and out.numel() == math.prod(shape)):
+        raise ValueError(f"out must be a contiguous CUDA tensor of {want} with {math.prod(shape)} elements")
     s = torch.cuda.current_stream(xyz.device).cuda_stream if stream is None else int(stream)
-    with torch.cuda.device(xyz.device):
-        rc = fn(xyz.data_ptr(), n, int(lmax), out.data_ptr(), layout_bits(layout, store, coords), s)
+    args = (xyz.data_ptr(), n, int(lmax), out.data_ptr(), layout_bits(layout, store, coords), s)
+    if xyz.device.index == torch.cuda.current_device():   # the usual case: no device switch (microseconds on launch-bound sizes)
+        rc = fn(*args)
+    else:
+        with torch.cuda.device(xyz.device):
+            rc = fn(*args)
     if rc != 0:
         raise ShError(rc, "sh_" + kind)
     return out
