@@ -363,6 +363,27 @@ __device__ __forceinline__ void evaluate_pair(const UnitVec& u0, const UnitVec& 
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
+// TMA bulk store shared -> global (cp.async.bulk, one bulk group per call site's commit).  The output is never re-read,
+// so its lines carry the L2 evict-first policy, like the st.global.cs of the LSU store paths: they leave L2 ahead of the
+// evict-last input prefetch and in the order they were written (SHB200_BULK_HINT = 0: no hint; measured in DESIGN.md section 6).
+#ifndef SHB200_BULK_HINT
+#define SHB200_BULK_HINT 1
+#endif
+__device__ __forceinline__ uint64_t l2_evict_first_policy() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void bulk_store(void* gdst, const void* ssrc, int bytes) {
+#if SHB200_BULK_HINT
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes),
+                 "l"(l2_evict_first_policy())
+                 : "memory");
+#else
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes) : "memory");
+#endif
+}
+
 // ------------------------------------------------------------------------------------------------
 // host side, shared by the translation units (defined in sh_abi.cu)
 extern std::atomic<int64_t> g_launches;   // kernels launched (sh_kernel_launch_count)

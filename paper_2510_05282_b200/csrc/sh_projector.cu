@@ -179,11 +179,9 @@ __global__ void __launch_bounds__(32 * SPLIT) sh_proj_aos_kernel(const double* _
         if (warp != 0) return;
         if (mode == PROJ_AOS_TILEBULK) {
             if (lane == 0)
-                asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(g), "r"(smem_u32(tile)), "r"(32 * ncols * 8) : "memory");
+                bulk_store(g, tile, 32 * ncols * 8);
         } else {
-            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(g + (int64_t)lane * ncols),
-                         "r"(smem_u32(tile + lane * pitch)), "r"(ncols * 8)
-                         : "memory");
+            bulk_store(g + (int64_t)lane * ncols, tile + lane * pitch, ncols * 8);
         }
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory is released when the CTA exits

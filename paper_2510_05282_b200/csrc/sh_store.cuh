@@ -115,9 +115,15 @@ __global__ void __launch_bounds__(32 * WARPS * SPLIT) sh_soa_tma_kernel(const do
     if constexpr (WARPS * SPLIT == 1) __syncwarp();
     else __syncthreads();
     if (threadIdx.x == 0) {
+#if SHB200_BULK_HINT
+        asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%1, %2}], [%3], %4;" ::"l"(&tmap), "r"((int)base), "r"(0),
+                     "r"(smem_u32(tile)), "l"(l2_evict_first_policy())
+                     : "memory");
+#else
         asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];" ::"l"(&tmap), "r"((int)base), "r"(0),
                      "r"(smem_u32(tile))
                      : "memory");
+#endif
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory is released when the CTA exits
     }
@@ -299,9 +305,7 @@ struct RowSink {
                 static_assert((LEN * sizeof(T)) % 16 == 0 && (BEGIN * sizeof(T)) % 16 == 0, "bulk granularity");
                 // generic-proxy staging stores -> visible to the async proxy, then one bulk copy for this row segment
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gout + i * SP + BEGIN),
-                             "r"(smem_u32(row)), "r"(LEN * (int)sizeof(T))
-                             : "memory");
+                bulk_store(gout + i * SP + BEGIN, row, LEN * (int)sizeof(T));
                 asm volatile("cp.async.bulk.commit_group;" ::: "memory");
                 if constexpr (L < LMAX) wait_reads();   // the row is reused by the next segment
             } else if constexpr (MODE == MODE_TILEBULK) {
@@ -311,9 +315,7 @@ struct RowSink {
                 const int bytes = rows * SP * (int)sizeof(T);
                 if (bytes % 16 == 0) {   // always for a full tile; a ragged last tile with an odd scalar count is copied by the warp
                     if (lane == 0) {
-                        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gout + base * SP),
-                                     "r"(smem_u32(tile)), "r"(bytes)
-                                     : "memory");
+                        bulk_store(gout + base * SP, tile, bytes);
                         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
                     }
                 } else {
