@@ -400,6 +400,25 @@ inline int launch_status() {
     return e == cudaSuccess ? SH_OK : cuda_fail(e);
 }
 
+// Dynamic shared memory above 48 KB is an opt-in per kernel AND per device (cudaFuncSetAttribute acts on the current device):
+// the largest size granted so far is remembered per device, so a process that drives several GPUs opts in on each.
+struct SmemOptIn {
+    std::atomic<size_t> granted[64];   // static storage: zero-initialised
+};
+template <class Kernel>
+inline int ensure_dynamic_smem(Kernel kern, size_t bytes, SmemOptIn& state) {
+    if (bytes <= 48 * 1024) return SH_OK;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    std::atomic<size_t>& slot = state.granted[dev & 63];
+    if (slot.load(std::memory_order_relaxed) >= bytes) return SH_OK;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e != cudaSuccess) return cuda_fail(e);
+    slot.store(bytes, std::memory_order_relaxed);
+    return SH_OK;
+}
+
 // cuTensorMapEncodeTiled through the runtime's driver entry point lookup (no link against libcuda); nullptr if unavailable
 using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
                                    const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);

@@ -448,12 +448,8 @@ template <int LMAX, int SPLIT>
 int launch_proj_aos_split(const double* xyz, int64_t n, const double* radial, const ProjPlan& plan, double* out, int pitch, int mode, size_t smem,
                           cudaStream_t st) {
     auto kern = sh_proj_aos_kernel<LMAX, SPLIT>;
-    static size_t smem_set = 0;   // the opt-in limit only ever grows
-    if (smem > 48 * 1024 && smem > smem_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return cuda_fail(e);
-        smem_set = smem;
-    }
+    static SmemOptIn opted_in;   // the opt-in limit only ever grows
+    if (const int rc = ensure_dynamic_smem(kern, smem, opted_in); rc != SH_OK) return rc;
     const int64_t ntiles = (n + 31) / 32;
     if (ntiles > 0x7fffffffLL) return SH_ERR_COUNT;
     kern<<<(unsigned)ntiles, 32 * SPLIT, smem, st>>>(xyz, n, radial, plan, out, pitch, mode, prefetch_plan(n, 32));
@@ -555,16 +551,12 @@ int launch_project(const double* xyz, int64_t n, const double* radial, const Pro
     const size_t slots_bytes = (size_t)4 * 32 * plan.first[shgen::LMAX_CAP + 1] * sizeof(double);
     constexpr size_t smem_max = (size_t)4 * (project_smem_doubles_per_warp<PROJ_NV>() + 32 * SH_MAX_PROJ) * sizeof(double);   // 86 KB
     const bool fast = tuned(SH_TUNE_PROJECT_FORM, 0) == 1;   // Horner / recurrence forms instead of the factorized ones
-    auto launch = [&](auto kern, size_t warp_doubles, bool& opted_in) -> int {
-        if (!opted_in) {
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
-            if (e != cudaSuccess) return cuda_fail(e);
-            opted_in = true;
-        }
+    auto launch = [&](auto kern, size_t warp_doubles, SmemOptIn& opted_in) -> int {
+        if (const int rc = ensure_dynamic_smem(kern, smem_max, opted_in); rc != SH_OK) return rc;
         kern<<<(unsigned)blocks, 128, (size_t)4 * warp_doubles * sizeof(double) + slots_bytes, st>>>(xyz, n, radial, plan, seg, w, nvec, partial);
         return SH_OK;
     };
-    static bool opted_in[4] = {false, false, false, false};
+    static SmemOptIn opted_in[4];
     int rc;
     if (nvec == 1) {
         rc = fast ? launch(sh_project_kernel<LMAX, 1, true>, project_smem_doubles_per_warp<1>(), opted_in[1])

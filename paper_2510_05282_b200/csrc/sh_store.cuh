@@ -418,16 +418,13 @@ int launch_soa_tma(const double* xyz, int64_t n, double* out, int coords, cudaSt
     const int64_t blocks = (n + PTS - 1) / PTS;
     constexpr size_t smem = (size_t)K * PTS * sizeof(double);
     static_assert(smem <= 227 * 1024, "tile exceeds shared memory");
-    auto launch = [&](auto kern, int split, bool& opted_in) -> int {
-        if (smem > 48 * 1024 && !opted_in) {
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e != cudaSuccess) return cuda_fail(e);
-            opted_in = true;
-        }
+    auto launch = [&](auto kern, int split, SmemOptIn& opted_in) -> int {
+        const int rc = ensure_dynamic_smem(kern, smem, opted_in);
+        if (rc != SH_OK) return rc;
         kern<<<(unsigned)blocks, PTS * split, smem, st>>>(xyz, n, tmap, coords, prefetch_plan(n, PTS));
         return launch_status();
     };
-    static bool opted_in[2] = {false, false};
+    static SmemOptIn opted_in[2];
     if constexpr (LMAX >= 4) {
         if (tuned(SH_TUNE_SOA_SPLIT, SHB200_SOA_SPLIT) >= 2) return launch(sh_soa_tma_kernel<LMAX, SOA_TMA_WARPS, 2>, 2, opted_in[1]);
     }
@@ -459,12 +456,12 @@ int launch_aos(const TI* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
     constexpr size_t smem = (size_t)WARPS * 32 * Sink::PITCH * sizeof(T);
     static_assert(smem <= 227 * 1024, "staging tile exceeds shared memory");
     auto kern = sh_aos_kernel<KIND, LMAX, T, TI, CAP, MODE, WARPS, ANGULAR>;
+    static SmemOptIn opted_in;
+    if (const int rc = ensure_dynamic_smem(kern, smem, opted_in); rc != SH_OK) return rc;
     static int ctas_per_sm = 0;   // idempotent cache of a pure function of the kernel
     if (!ctas_per_sm) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return cuda_fail(e);
         int occ = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, WARPS * 32, smem);
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, WARPS * 32, smem);
         if (e != cudaSuccess) return cuda_fail(e);
         ctas_per_sm = occ > 0 ? occ : 1;
     }
