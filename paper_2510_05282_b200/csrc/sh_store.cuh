@@ -88,17 +88,18 @@ struct TileSink {
 };
 
 // SPLIT warps share each 32-point group of the tile, each evaluating part of the l-blocks (block_part in sh_core.cuh)
-template <int LMAX, int WARPS, int SPLIT>
+template <int LMAX, int WARPS, int SPLIT, bool ANGULAR>
 __global__ void __launch_bounds__(32 * WARPS * SPLIT) sh_soa_tma_kernel(const double* __restrict__ xyz, int64_t n, const __grid_constant__ CUtensorMap tmap,
                                                                          int coords, InputPrefetch pf) {
     constexpr int PTS = 32 * WARPS;
     extern __shared__ __align__(128) unsigned char smem_tile[];
-    prefetch_input_window(xyz, n * 24, (int64_t)PTS * 24, pf);
+    constexpr int IN_BYTES = (ANGULAR ? 2 : 3) * sizeof(double);
+    prefetch_input_window(xyz, n * IN_BYTES, (int64_t)PTS * IN_BYTES, pf);
     double* tile = reinterpret_cast<double*>(smem_tile);
     const int p = SPLIT == 1 ? threadIdx.x : threadIdx.x % PTS;   // point of the tile
     const int64_t base = (int64_t)blockIdx.x * PTS, i = base + p;
     if (i < n) {
-        RawPoint<double> pt;
+        RawPoint<double, ANGULAR> pt;
         pt.load(xyz, i);
         TileSink<PTS> sink{tile + p};
         const UnitVec u = pt.unit(coords);
@@ -402,7 +403,7 @@ int launch_soa(const TI* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
 
 // SoA through the tensor unit: `out` as a 2-D tensor [K][n] of fp64 (row pitch 8n bytes must be a multiple of 16: n even),
 // box {points per tile, K}.  Returns SH_ERR_ALIGNMENT when this launch cannot use the path (the caller then takes sh_soa_kernel).
-template <int LMAX>
+template <int LMAX, bool ANGULAR = false>
 int launch_soa_tma(const double* xyz, int64_t n, double* out, int coords, cudaStream_t st) {
     constexpr int K = (LMAX + 1) * (LMAX + 1);
     constexpr int PTS = 32 * SOA_TMA_WARPS;
@@ -426,9 +427,9 @@ int launch_soa_tma(const double* xyz, int64_t n, double* out, int coords, cudaSt
     };
     static SmemOptIn opted_in[2];
     if constexpr (LMAX >= 4) {
-        if (tuned(SH_TUNE_SOA_SPLIT, SHB200_SOA_SPLIT) >= 2) return launch(sh_soa_tma_kernel<LMAX, SOA_TMA_WARPS, 2>, 2, opted_in[1]);
+        if (tuned(SH_TUNE_SOA_SPLIT, SHB200_SOA_SPLIT) >= 2) return launch(sh_soa_tma_kernel<LMAX, SOA_TMA_WARPS, 2, ANGULAR>, 2, opted_in[1]);
     }
-    return launch(sh_soa_tma_kernel<LMAX, SOA_TMA_WARPS, 1>, 1, opted_in[0]);
+    return launch(sh_soa_tma_kernel<LMAX, SOA_TMA_WARPS, 1, ANGULAR>, 1, opted_in[0]);
 }
 
 // staging capacity per row, in scalars: whole rows for real (800 B at lmax = 9) and complex (1600 B);
@@ -493,9 +494,15 @@ int dispatch_lmax(const TI* xyz, int64_t n, T* out, int layout, int path, int co
     constexpr int SP = scalars_per_point(KIND, LMAX);
     constexpr bool F32 = std::is_same<T, float>::value && KIND == KIND_REAL;
     if (coords == SH_COORDS_ANGULAR) {
-        // angular front end: trigonometry dominates; it is served by the generic store paths only (scalar SoA stores,
-        // AoS staging + coalesced copy-out), which are valid for every alignment
+        // angular front end: served by the generic store paths (scalar SoA stores, AoS staging + coalesced copy-out), which
+        // are valid for every alignment -- except sh_real SoA, which takes the tensor-store path where `out` allows it
         if (path == SH_STORE_BULK) return SH_ERR_ALIGNMENT;
+        if constexpr (KIND == KIND_REAL && std::is_same<T, double>::value) {
+            if (layout == SH_LAYOUT_SOA && path == SH_STORE_AUTO && tuned(SH_TUNE_SOA_TMA, 0) != 1) {   // the tensor-store path of sh_real SoA
+                const int rc = launch_soa_tma<LMAX, true>(reinterpret_cast<const double*>(xyz), n, reinterpret_cast<double*>(out), coords, st);
+                if (rc != SH_ERR_ALIGNMENT) return rc;
+            }
+        }
         if (layout == SH_LAYOUT_SOA) return launch_soa<KIND, LMAX, T, TI, 8, true>(xyz, n, out, coords, st);
         return launch_aos<KIND, LMAX, T, TI, MODE_PLAIN, true>(xyz, n, out, coords, st);
     }
