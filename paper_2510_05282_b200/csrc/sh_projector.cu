@@ -41,7 +41,7 @@ struct RadialPos {
 // Radial values of EVERY channel slot at this lane's point, computed up front and parked in shared memory as
 // fs[slot*32 + lane] (times `scale`).  The table loads of different slots are independent, so their latencies overlap;
 // loaded one l-block at a time instead, a warp pays one dependent L2 round trip per channel (the staging tiles leave
-// little L1), which is what bounds the low-occupancy staging kernels (AoS sh_projectors 0.41 -> see DESIGN.md section 6).
+// little L1).  sh_project uses this; sh_proj_aos_kernel shares the slots among the warps of its tile the same way.
 __device__ __forceinline__ void stage_radial(const RadialPos& pos, const double* __restrict__ radial, const ProjPlan& plan, double* fs, int lane,
                                              double scale) {
     const int nslots = plan.first[shgen::LMAX_CAP + 1];
