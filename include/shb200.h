@@ -169,11 +169,11 @@ enum {
     SH_TUNE_AOS_TILES_PER_WARP = 1, /* consecutive 32-point tiles one warp of the AoS kernels processes */
     SH_TUNE_PREFETCH_WINDOW_POINTS = 2, /* points per burst of the L2 input prefetch (default 262144); 1 = prefetch off */
     SH_TUNE_PROJ_AOS_MODE = 3,      /* sh_projectors AoS copy-out: 1 = warp copy, 2 = one bulk copy per row, 3 = one per tile (when possible) */
-    SH_TUNE_SOA_TMA = 4,            /* sh_real SoA through one TMA tensor store per 128-point tile: 0 = when possible (default), 1 = never */
+    SH_TUNE_SOA_TMA = 4,            /* sh_real / sh_real_f32 SoA through one TMA tensor store per tile of 1 KB rows (128 / 256 points): 0 = when possible (default), 1 = never */
     SH_TUNE_PROJECT_FORM = 5,       /* sh_project polynomials: 0 = the factorized forms of every other call (default); 1 = Horner in z^2 for the
                                        polar factors and (x + iy)^m by recurrence: ~35 % fewer FP64 instructions, same tolerance */
     SH_TUNE_PROJ_AOS_SPLIT = 6,     /* sh_projectors AoS, lmax >= 4: warps that share one 32-point tile, each evaluating part of the l-blocks: 1, 2 (default) or 4 */
-    SH_TUNE_SOA_SPLIT = 7,          /* sh_real SoA tensor-store path, lmax >= 4: warps that share a 32-point group of the tile, each evaluating part of the l-blocks: 1 or 2 (default) */
+    SH_TUNE_SOA_SPLIT = 7,          /* sh_real / sh_real_f32 SoA tensor-store path, lmax >= 4: warps that share a 32-point group of the tile, each evaluating part of the l-blocks: 1 or 2 (default) */
     SH_TUNE_COUNT = 8
 };
 int sh_set_tuning(int knob, int value);

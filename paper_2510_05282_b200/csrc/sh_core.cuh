@@ -257,9 +257,9 @@ constexpr int part_mmax() {   // largest m the part's blocks need
     return m;
 }
 
-template <int LMAX, int SPLIT, int PART, class O, class Sink>
-__device__ __forceinline__ void eval_real_part(double x, double y, double z, O origin, Sink& sink) {
-    const Azim<part_mmax<SPLIT, PART, LMAX>(), double> az(x, y);
+template <int LMAX, int SPLIT, int PART, typename T, class O, class Sink>
+__device__ __forceinline__ void eval_real_part(T x, T y, T z, O origin, Sink& sink) {
+    const Azim<part_mmax<SPLIT, PART, LMAX>(), T> az(x, y);
     static_for<0, LMAX + 1>([&](auto lc) {
         constexpr int L = decltype(lc)::value;
         if constexpr (block_part<SPLIT>(L) == PART) real_block<L>(az, z, origin, sink);

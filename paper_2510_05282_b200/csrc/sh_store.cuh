@@ -79,36 +79,38 @@ constexpr int SOA_TMA_WARPS = SHB200_SOA_TMA_WARPS;
 #define SHB200_SOA_SPLIT 2
 #endif
 
-template <int PTS>
+template <int PTS, typename T = double>
 struct TileSink {
-    double* col;   // tile + this thread's point
-    template <int K> __device__ __forceinline__ void put1(double v) { col[K * PTS] = v; }
+    T* col;   // tile + this thread's point
+    template <int K> __device__ __forceinline__ void put1(T v) { col[K * PTS] = v; }
     template <int L> __device__ __forceinline__ void end_l() {}
-    template <int L> __device__ __forceinline__ void polar(const double (&)[L + 1]) {}
+    template <int L> __device__ __forceinline__ void polar(const T (&)[L + 1]) {}
 };
 
 // SPLIT warps share each 32-point group of the tile, each evaluating part of the l-blocks (block_part in sh_core.cuh)
-template <int LMAX, int WARPS, int SPLIT, bool ANGULAR>
-__global__ void __launch_bounds__(32 * WARPS * SPLIT) sh_soa_tma_kernel(const double* __restrict__ xyz, int64_t n, const __grid_constant__ CUtensorMap tmap,
-                                                                         int coords, InputPrefetch pf) {
+// T = float (sh_real_f32): the same kernel on 256-point tiles (rows of 1 KB again), fp64 normalization, fp32 polynomials.
+template <typename T, int LMAX, int WARPS, int SPLIT, bool ANGULAR>
+__global__ void __launch_bounds__(32 * WARPS * SPLIT, WARPS * SPLIT > 8 ? 2 : 1) sh_soa_tma_kernel(const T* __restrict__ xyz, int64_t n,
+                                                                                                  const __grid_constant__ CUtensorMap tmap, int coords,
+                                                                                                  InputPrefetch pf) {
     constexpr int PTS = 32 * WARPS;
     extern __shared__ __align__(128) unsigned char smem_tile[];
-    constexpr int IN_BYTES = (ANGULAR ? 2 : 3) * sizeof(double);
+    constexpr int IN_BYTES = (ANGULAR ? 2 : 3) * sizeof(T);
     prefetch_input_window(xyz, n * IN_BYTES, (int64_t)PTS * IN_BYTES, pf);
-    double* tile = reinterpret_cast<double*>(smem_tile);
+    T* tile = reinterpret_cast<T*>(smem_tile);
     const int p = SPLIT == 1 ? threadIdx.x : threadIdx.x % PTS;   // point of the tile
     const int64_t base = (int64_t)blockIdx.x * PTS, i = base + p;
     if (i < n) {
-        RawPoint<double, ANGULAR> pt;
+        RawPoint<T, ANGULAR> pt;
         pt.load(xyz, i);
-        TileSink<PTS> sink{tile + p};
+        TileSink<PTS, T> sink{tile + p};
         const UnitVec u = pt.unit(coords);
-        if constexpr (SPLIT == 1) evaluate<KIND_REAL, LMAX, double>(u, sink);
+        if constexpr (SPLIT == 1) evaluate<KIND_REAL, LMAX, T>(u, sink);
         else {
             const int part = threadIdx.x / PTS;   // warp-uniform
             static_for<0, SPLIT>([&](auto pc) {
                 constexpr int PART = decltype(pc)::value;
-                if (part == PART) eval_real_part<LMAX, SPLIT, PART>(u.x, u.y, u.z, u.origin, sink);
+                if (part == PART) eval_real_part<LMAX, SPLIT, PART>((T)u.x, (T)u.y, (T)u.z, u.origin, sink);   // fp32: rounded once, after the fp64 normalization
             });
         }
     }
@@ -401,23 +403,25 @@ int launch_soa(const TI* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
     return launch_status();
 }
 
-// SoA through the tensor unit: `out` as a 2-D tensor [K][n] of fp64 (row pitch 8n bytes must be a multiple of 16: n even),
-// box {points per tile, K}.  Returns SH_ERR_ALIGNMENT when this launch cannot use the path (the caller then takes sh_soa_kernel).
-template <int LMAX, bool ANGULAR = false>
-int launch_soa_tma(const double* xyz, int64_t n, double* out, int coords, cudaStream_t st) {
+// SoA through the tensor unit: `out` as a 2-D tensor [K][n] of fp64 / fp32 (row pitch must be a multiple of 16 bytes: n even /
+// a multiple of 4), box {points per tile, K}, tiles of 1 KB rows (128 / 256 points).  Returns SH_ERR_ALIGNMENT when this launch
+// cannot use the path (the caller then takes the LSU-store kernels).
+template <int LMAX, bool ANGULAR = false, typename T = double>
+int launch_soa_tma(const T* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
     constexpr int K = (LMAX + 1) * (LMAX + 1);
-    constexpr int PTS = 32 * SOA_TMA_WARPS;
+    constexpr int TMA_WARPS = SOA_TMA_WARPS * (int)(sizeof(double) / sizeof(T));
+    constexpr int PTS = 32 * TMA_WARPS;
     EncodeTiledFn enc = encode_tiled();
-    if (!enc || (n & 1) || n < PTS || n > 0x7fffff00LL || !aligned(out, 16)) return SH_ERR_ALIGNMENT;
+    if (!enc || (n * sizeof(T)) % 16 != 0 || n < PTS || n > 0x7fffff00LL || !aligned(out, 16)) return SH_ERR_ALIGNMENT;
     CUtensorMap tmap;
     const cuuint64_t gdim[2] = {(cuuint64_t)n, (cuuint64_t)K};
-    const cuuint64_t gstride[1] = {(cuuint64_t)n * sizeof(double)};
+    const cuuint64_t gstride[1] = {(cuuint64_t)n * sizeof(T)};
     const cuuint32_t box[2] = {PTS, (cuuint32_t)K}, estride[2] = {1, 1};
-    if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, out, gdim, gstride, box, estride, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+    if (enc(&tmap, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, out, gdim, gstride, box, estride, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
             CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return SH_ERR_ALIGNMENT;
     const int64_t blocks = (n + PTS - 1) / PTS;
-    constexpr size_t smem = (size_t)K * PTS * sizeof(double);
+    constexpr size_t smem = (size_t)K * PTS * sizeof(T);
     static_assert(smem <= 227 * 1024, "tile exceeds shared memory");
     auto launch = [&](auto kern, int split, SmemOptIn& opted_in) -> int {
         const int rc = ensure_dynamic_smem(kern, smem, opted_in);
@@ -427,9 +431,9 @@ int launch_soa_tma(const double* xyz, int64_t n, double* out, int coords, cudaSt
     };
     static SmemOptIn opted_in[2];
     if constexpr (LMAX >= 4) {
-        if (tuned(SH_TUNE_SOA_SPLIT, SHB200_SOA_SPLIT) >= 2) return launch(sh_soa_tma_kernel<LMAX, SOA_TMA_WARPS, 2, ANGULAR>, 2, opted_in[1]);
+        if (tuned(SH_TUNE_SOA_SPLIT, SHB200_SOA_SPLIT) >= 2) return launch(sh_soa_tma_kernel<T, LMAX, TMA_WARPS, 2, ANGULAR>, 2, opted_in[1]);
     }
-    return launch(sh_soa_tma_kernel<LMAX, SOA_TMA_WARPS, 1, ANGULAR>, 1, opted_in[0]);
+    return launch(sh_soa_tma_kernel<T, LMAX, TMA_WARPS, 1, ANGULAR>, 1, opted_in[0]);
 }
 
 // staging capacity per row, in scalars: whole rows for real (800 B at lmax = 9) and complex (1600 B);
@@ -517,6 +521,11 @@ int dispatch_lmax(const TI* xyz, int64_t n, T* out, int layout, int path, int co
             }
         }
         if constexpr (F32) {
+            // one tensor store per 256-point tile where `out` allows it (16-byte aligned, n a multiple of 4)
+            if (path == SH_STORE_AUTO && tuned(SH_TUNE_SOA_TMA, 0) != 1) {
+                const int rc = launch_soa_tma<LMAX, false, float>(reinterpret_cast<const float*>(xyz), n, reinterpret_cast<float*>(out), coords, st);
+                if (rc != SH_ERR_ALIGNMENT) return rc;
+            }
             // two adjacent points per thread (packed fp32, 8-byte stores) when every plane keeps 8-byte alignment
             if (n >= 2 && n % 2 == 0 && aligned(out, 8) && aligned(xyz, 8) && path != SH_STORE_DIRECT)
                 return launch_soa_pair<LMAX>(reinterpret_cast<const float*>(xyz), n, reinterpret_cast<float*>(out), coords, st);

@@ -195,14 +195,28 @@ def test_near_pole_points(sh, oracle_mod):
 
 
 def test_fp32_pair_and_scalar_paths(sh, oracle_mod, cube_points):
-    """fp32 SoA: even n and 8-byte aligned out -> two-points-per-thread packed-fp32 kernel; otherwise scalar kernel."""
+    """fp32 SoA: n a multiple of 4, n >= 256 and a 16-byte aligned out -> one tensor store per 256-point tile (one or two
+    warps per 32-point group); else even n and 8-byte aligned out (or `soa_tma` = 1) -> two-points-per-thread packed-fp32
+    kernel; otherwise the scalar LSU-store kernel.  The tensor-store and scalar kernels run the same fp32 arithmetic."""
     x32 = cube_points.astype(np.float32)
-    for n in (10008, 10007, 3, 2, 1):
+    for n in (10008, 10007, 10006, 256, 252, 3, 2, 1):
+        want = oracle_mod.real(x32[:n].astype(np.float64), 9)
         for mis in (0, 1):
             for store in ("auto", "direct"):
-                got = gpu_eval(sh, "real_f32", x32[:n], 9, "soa", store, misalign=mis)
-                want = oracle_mod.real(x32[:n].astype(np.float64), 9)
-                assert max_err(got.astype(np.float64), want) <= TOL32, (n, mis, store)
+                for tma_off, split in ((0, 1), (0, 2), (1, 0)):
+                    sh.set_tuning("soa_tma", tma_off)
+                    sh.set_tuning("soa_split", split)
+                    try:
+                        got = gpu_eval(sh, "real_f32", x32[:n], 9, "soa", store, misalign=mis)
+                    finally:
+                        sh.set_tuning("soa_tma", 0)
+                        sh.set_tuning("soa_split", 0)
+                    assert max_err(got.astype(np.float64), want) <= TOL32, (n, mis, store, tma_off, split)
+                    if store == "direct":
+                        scalar = got
+                    elif tma_off == 0 and n % 4 == 0 and n >= 256 and mis == 0:
+                        tensor = got
+        assert n % 4 or n < 256 or np.array_equal(tensor, scalar), n
 
 
 # ----------------------------------------------------------------------------- front ends (P:69)
