@@ -89,8 +89,11 @@ struct TileSink {
 
 // SPLIT warps share each 32-point group of the tile, each evaluating part of the l-blocks (block_part in sh_core.cuh)
 // T = float (sh_real_f32): the same kernel on 256-point tiles (rows of 1 KB again), fp64 normalization, fp32 polynomials.
+// Two CTAs per SM is what the 102 KB tile allows.  fp32 (512 threads with SPLIT = 2) needs the register cap of minBlocks = 2;
+// for fp64 minBlocks stays unspecified (0): given a cap, ptxas spends registers up to it (64 -> 120 at minBlocks = 2, and 148,
+// i.e. ONE resident CTA and 0.41 instead of 0.24 ms, at minBlocks = 1).
 template <typename T, int LMAX, int WARPS, int SPLIT, bool ANGULAR>
-__global__ void __launch_bounds__(32 * WARPS * SPLIT, WARPS * SPLIT > 8 ? 2 : 1) sh_soa_tma_kernel(const T* __restrict__ xyz, int64_t n,
+__global__ void __launch_bounds__(32 * WARPS * SPLIT, sizeof(T) == 4 ? 2 : 0) sh_soa_tma_kernel(const T* __restrict__ xyz, int64_t n,
                                                                                                   const __grid_constant__ CUtensorMap tmap, int coords,
                                                                                                   InputPrefetch pf) {
     constexpr int PTS = 32 * WARPS;
