@@ -9,8 +9,12 @@ Output buffers (1.68 GB each) are far larger than L2 (126 MB); inputs and output
 replicas so nothing is re-read from L2 between timed iterations.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-N > 1 is launched by torchrun (one rank per GPU); points are independent, so ranks run the same-size
-grid with no data-path collective ("weak" scaling); timing is the max over ranks of CUDA-event time.
+N > 1 is launched by torchrun (one rank per GPU); points are independent, so the job is a contiguous point-range
+partition (inputs.shard_range) of N grids, one grid per rank, with no data-path collective ("weak" scaling);
+timing is the max over ranks of CUDA-event time.
+
+Ceilings are measured in the same run from committed code (csrc/sh_peaks.cu): write-only fills in the kernels' own
+store patterns (`roofline.write_fill_gbs`) and a DFMA chain (the `alu` peak of the FP64-bound fused projection).
 """
 from __future__ import annotations
 
@@ -45,8 +49,10 @@ def measured_peak():
 
 
 def ncu_traffic(kernel_key: str):
-    """Per-launch DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel from the committed ncu
-    summary profiles/ncu_traffic.csv (see profiles/r1_launches.md for the commands), or None."""
+    """Per-launch DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of a kernel family from the committed ncu
+    summaries (profiles/ncu_traffic.csv, one row per family, copied from the `ncu --set full` captures named in
+    profiles/r2_launches.md), or None.  A profiler counter cannot be read inside an unprofiled run: this is the committed
+    measurement of the same kernel on the same workload, not a live one."""
     try:
         import csv
 
@@ -110,6 +116,91 @@ class ClockSampler:
         return out
 
 
+def ceilings(dev, sampler_index=None):
+    """The two ceilings SURVEY.md asks the build to measure (section 6: an FP64 DFMA peak; section 8(d) denominator (ii): a
+    write-only fill "measured in the same run"), from committed code (csrc/sh_peaks.cu), with the bench's own discipline:
+    CUDA events on the launching stream, 3 warm-ups, median of 20, two rotating 1.68 GB buffers (far larger than L2).
+      write_fill_gbs.flat        one flat stream of 32-byte evict-first stores
+      write_fill_gbs.bulk_tiles  contiguous 25.6 KB tiles, one TMA bulk copy each        (the AoS kernels' store pattern)
+      write_fill_gbs.soa_planes  [100][N] planes, one TMA tensor store per 128-point tile (the SoA kernels' store pattern)
+      write_fill_gbs.memset      cudaMemsetAsync through torch (`zero_`), the driver's own fill
+      fp64_lane_ginstr_s         DFMA chains at full occupancy for >= 1 s (so the clock is the power-capped one), with the SM clock sampled meanwhile."""
+    import torch
+    from paper_2510_05282_b200 import peaks
+
+    n = 128 ** 3
+    bufs = [torch.empty((K, n), dtype=torch.float64, device=dev) for _ in range(2)]
+    nbytes = bufs[0].numel() * 8
+
+    def med(fn):
+        for it in range(3):
+            fn(bufs[it % 2])
+        torch.cuda.synchronize()
+        ts = []
+        for it in range(20):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn(bufs[it % 2])
+            b.record()
+            b.synchronize()
+            ts.append(a.elapsed_time(b))
+        return nbytes / (statistics.median(ts) * 1e-3) / 1e9
+
+    fills = {
+        "flat": med(peaks.fill_flat),
+        "bulk_tiles": med(lambda o: peaks.fill_bulk_tiles(o, 32 * K * 8)),
+        "soa_planes": med(lambda o: peaks.fill_soa_planes(o, 128, K)),
+        "memset": med(lambda o: o.zero_()),
+    }
+    del bufs
+    torch.cuda.empty_cache()
+    # FP64 pipe: 8 CTAs of 256 threads per SM (full occupancy), launches of ~20 ms back to back for >= 1 s
+    sink = torch.zeros(8, dtype=torch.float64, device=dev)
+    blocks = N_SMS * 8
+    iters = 1 << 16
+    peaks.dfma(sink, iters, blocks)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(sampler_index) if sampler_index is not None else None
+    wall0 = time.time()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    lane_instr = 0
+    launches = 0
+    while True:
+        for _ in range(10):
+            lane_instr += peaks.dfma(sink, iters, blocks)
+            launches += 1
+        torch.cuda.synchronize()
+        if time.time() - wall0 >= 1.0:
+            break
+    b.record()
+    torch.cuda.synchronize()
+    ms = a.elapsed_time(b)
+    clocks = sampler.stop(wall0, time.time()) if sampler else None
+    ginstr = lane_instr / (ms * 1e-3) / 1e9
+    return {
+        "write_fill_gbs": fills,
+        "fp64_lane_ginstr_s": ginstr, "fp64_tflops_dfma": 2 * ginstr / 1e3,
+        "fp64_measure": {"ms": ms, "launches": launches, "sm_mhz": clocks and clocks.get("sm_mhz"), "reasons": clocks and clocks.get("reasons"),
+                         "lanes_per_sm_per_clk_at_sampled_clock": (ginstr * 1e3 / (N_SMS * clocks["sm_mhz"]) if clocks and clocks.get("sm_mhz") else None)},
+        "how": "csrc/sh_peaks.cu through paper_2510_05282_b200/peaks.py, CUDA events, same run",
+    }
+
+
+def hbm_roofline(kernel, alg_bytes, written_bytes, ms, peak, peak_src, ceil, pattern, traffic_key=None):
+    """`roofline` block of an HBM-bound launch: achieved = algorithmic bytes (in + out) per launch / average launch time against
+    the driver-measured copy peak, plus the written bytes against the write-only fill ceiling of the kernel's own store pattern."""
+    achieved = alg_bytes / (ms * 1e-3) / 1e9
+    wr = written_bytes / (ms * 1e-3) / 1e9
+    blk = {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+           "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": ms, "achieved_write": wr,
+           "traffic": ncu_traffic(traffic_key) if traffic_key else None}
+    if ceil:
+        fill = ceil["write_fill_gbs"][pattern]
+        blk.update({"write_fill_gbs": fill, "write_fill_pattern": pattern, "frac_of_write_fill": wr / fill})
+    return blk
+
+
 def grid_points():
     from paper_2510_05282_b200 import inputs
 
@@ -143,6 +234,36 @@ def cpu_baseline(pts, target_seconds=12.0):
         "sample": f"first {m} points of the 128^3 grid, lmax=9 real, long double, one evaluation, {dt:.2f} s",
         "value_one_thread": m1 * K / dt1 / 1e9, "sample_one_thread": f"first {m1} points, {dt1:.2f} s",
     }
+
+
+def cpu_method(pts):
+    """The paper's own CPU scheme on this box's host cores: the generated factorized fp64 formulas compiled for
+    the host (baseline/sh_cpu_method.cpp), every l <= 9 at every grid point, stored as AoS [N][100]; all cores and one thread,
+    plus the compute-only (accumulate, never store: P:140) rate that is comparable with the paper's Table I."""
+    import baseline
+
+    baseline.build()
+    n = len(pts)
+    out = np.empty((n, K))
+    res = {"unit": UNIT, "kind": "paper method: generated factorized formulas, fp64, host build (baseline/sh_cpu_method.cpp)",
+           "sample": f"all {n} grid points, lmax=9 real, AoS store, second of two passes (the first touches the pages)"}
+    for label, threads in (("", 0), ("_one_thread", 1)):
+        baseline.set_threads(threads)
+        m = n if threads == 0 else n // 8
+        baseline.real(pts[:m], LMAX, out=out[:m])
+        t0 = time.perf_counter()
+        baseline.real(pts[:m], LMAX, out=out[:m])
+        dt = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        baseline.accumulate_l9(pts[:m])
+        dta = time.perf_counter() - t0
+        res["value" + label] = m * K / dt / 1e9
+        res["value_accumulate_only" + label] = m * K / dta / 1e9
+        if threads == 0:
+            res["cores"] = baseline.threads()
+    baseline.set_threads(0)
+    res["sample_one_thread"] = f"first {n // 8} grid points"
+    return res
 
 
 def run_reference(args):
@@ -184,7 +305,7 @@ def run_reference(args):
     print(json.dumps(line))
 
 
-def extra_configs(sh, dev, only=None):
+def extra_configs(sh, dev, only=None, ceil=None):
     """The other BASELINE.json configs, timed with CUDA events outside the headline's timed region (context, not `value`).
     `only`: run just the cases whose name contains this substring (what the ncu captures under profiles/ use)."""
     import torch
@@ -227,6 +348,7 @@ def extra_configs(sh, dev, only=None):
         return a.elapsed_time(b) / reps
 
     res = {}
+    peak, peak_src = measured_peak()
     # the paper's three front ends (Table I) on the headline workload, SoA
     grid = inputs.config3_full_grid()
     rr = np.linalg.norm(grid, axis=1)
@@ -239,7 +361,9 @@ def extra_configs(sh, dev, only=None):
             continue
         x = torch.from_numpy(arr).to(dev)
         ms = timed(lambda: sh.sh_real(x, LMAX, out=out, layout="soa", coords=coords), 20)
-        res[f"config3 real l9 SoA front end {coords}"] = {"ms": ms, "write_GBps": len(grid) * K * 8 / ms / 1e6, "G_values_per_s": len(grid) * K / ms / 1e6}
+        res[f"config3 real l9 SoA front end {coords}"] = {
+            "ms": ms, "write_GBps": len(grid) * K * 8 / ms / 1e6, "G_values_per_s": len(grid) * K / ms / 1e6,
+            "roofline": hbm_roofline(f"sh_real lmax=9 SoA, {coords} input", len(grid) * (arr.shape[1] * 8 + 8 * K), len(grid) * 8 * K, ms, peak, peak_src, ceil, "soa_planes")}
         del x
     del out
     cases = [
@@ -271,31 +395,38 @@ def extra_configs(sh, dev, only=None):
                 "ms": ms, "write_GBps": n * per_point * esize / ms / 1e6,
                 "G_values_per_s": n * per_point / values / ms / 1e6,
             }
+            if n >= (1 << 18):   # HBM-bound sizes: algorithmic bytes = xyz in + every scalar out
+                res[f"{name} {layout}"]["roofline"] = hbm_roofline(
+                    f"sh_{kind} lmax={lmax} {layout}", n * (3 * esize + per_point * esize), n * per_point * esize, ms, peak, peak_src, ceil,
+                    "soa_planes" if layout == "soa" else "bulk_tiles", traffic_key=f"{kind}_{layout}")
             if n < (1 << 18):   # launch-bound sizes: also as CUDA-graph replays
                 res[f"{name} {layout}"]["ms_in_cuda_graph"] = timed_graph(lambda: fn(x, lmax, out=out, layout=layout), 100)
             del out
         del x
         torch.cuda.empty_cache()
-    res.update(projector_cases(sh, dev, timed, timed_graph, want))
+    res.update(projector_cases(sh, dev, timed, timed_graph, want, ceil))
     return res
 
 
-# FP64 pipe peak for the ALU-bound fused projection: 64 FP64 lanes per SM per clock (B300_MICROARCH.md
-# unit counts; confirmed here by a DFMA microbenchmark: 36.7 TFLOP/s = 148 x 64 x 2 x 1.94 GHz), one DADD/DMUL/DFMA = one
-# lane-slot.  Peak = 148 SMs x 64 lanes x clock; the clock is the nvidia-smi maximum (1965 MHz), so power-capped runs read low.
+# FP64 pipe peak for the ALU-bound fused projection: one DADD/DMUL/DFMA = one lane-slot of the FP64 pipe.
+# The peak is MEASURED in the same run (ceilings(): DFMA chains at full occupancy for >= 1 s, csrc/sh_peaks.cu); the nominal
+# figure 148 SMs x 64 lanes x 1.965 GHz (B300_MICROARCH.md unit counts x the nvidia-smi maximum clock) is printed beside it.
 FP64_LANES_PER_SM = 64
 N_SMS = 148
 SM_MAX_GHZ = 1.965
 
 
-def projector_cases(sh, dev, timed, timed_graph, want):
+def projector_cases(sh, dev, timed, timed_graph, want, ceil=None):
     """Fused projector consumer: sh_projectors (stores only the requested columns) and sh_project
     (contraction with weight vectors; writes nothing per point, FP64-pipe bound)."""
     import torch
     from paper_2510_05282_b200 import inputs
 
     res = {}
-    peak_ginstr = N_SMS * FP64_LANES_PER_SM * SM_MAX_GHZ  # G FP64 lane-instructions/s
+    nominal_ginstr = N_SMS * FP64_LANES_PER_SM * SM_MAX_GHZ  # G FP64 lane-instructions/s
+    peak_ginstr = ceil["fp64_lane_ginstr_s"] if ceil else nominal_ginstr
+    peak_src = "measured in this run (DFMA chains, csrc/sh_peaks.cu)" if ceil else "nominal 148 SMs x 64 lanes x 1.965 GHz"
+    hbm_peak, hbm_src = measured_peak()
     work = [
         # name, points, (lmax, per_l, cutoff, dr), volume element
         ("config2 grid l3 x2 channels (32 cols)", inputs.config2_projector_grid(), (3, 2, 3.0, 0.01), 1e-3),
@@ -316,13 +447,12 @@ def projector_cases(sh, dev, timed, timed_graph, want):
             out = torch.empty((ncols, n) if layout == "soa" else (n, ncols), dtype=torch.float64, device=dev)
             ms = timed(lambda: sh.sh_projectors(x, proj_l, t, dr, out=out, layout=layout), reps)
             res[f"projectors {layout} {name}"] = {"ms": ms, "write_GBps": n * ncols * 8 / ms / 1e6, "G_values_per_s": n * ncols / ms / 1e6}
+            if n >= (1 << 18):
+                res[f"projectors {layout} {name}"]["roofline"] = hbm_roofline(
+                    f"sh_projectors {layout}, {ncols} columns", n * (24 + 8 * ncols), n * 8 * ncols, ms, hbm_peak, hbm_src, ceil,
+                    "soa_planes" if layout == "soa" else "bulk_tiles", traffic_key=f"projectors_{layout}")
             if n < (1 << 18):
                 res[f"projectors {layout} {name}"]["ms_in_cuda_graph"] = timed_graph(lambda: sh.sh_projectors(x, proj_l, t, dr, out=out, layout=layout), 100)
-            if layout == "aos" and os.environ.get("SHB200_BENCH_SWEEP"):
-                for mode in (1, 2, 3):
-                    sh.set_tuning("proj_aos_mode", mode)
-                    res[f"projectors {layout} {name}"][f"ms_mode{mode}"] = timed(lambda: sh.sh_projectors(x, proj_l, t, dr, out=out, layout=layout), reps)
-                sh.set_tuning("proj_aos_mode", 0)
             del out
         for nvec in (1, 4):
             if not want(f"project nvec={nvec} {name}"):
@@ -340,8 +470,8 @@ def projector_cases(sh, dev, timed, timed_graph, want):
                 "ms": ms, "G_points_per_s": n / ms / 1e6, "G_values_per_s": n * ncols * nvec / ms / 1e6,
                 "read_GBps": n * (24 + 8 * nvec) / ms / 1e6,
                 "roofline": {"bound": "alu", "unit": "G FP64 lane-instr/s", "achieved": n * fp64_per_point / ms / 1e6,
-                             "peak": peak_ginstr, "frac": n * fp64_per_point / ms / 1e6 / peak_ginstr,
-                             "fp64_instr_per_point": fp64_per_point},
+                             "peak": peak_ginstr, "frac": n * fp64_per_point / ms / 1e6 / peak_ginstr, "peak_source": peak_src,
+                             "peak_nominal": nominal_ginstr, "fp64_instr_per_point": fp64_per_point},
             }
             if n < (1 << 18):
                 res[f"project nvec={nvec} {name}"].update({"ms": ms_py, "ms_in_cuda_graph": ms})
@@ -393,7 +523,13 @@ def run_ours(args):
             dist.barrier()
 
     sampler = ClockSampler(local) if rank == 0 else None  # started early: nvidia-smi needs ~0.2 s to come up
-    pts = grid_points()
+    grid = grid_points()
+    # the job is `world` grids laid end to end, cut into contiguous point ranges (inputs.shard_range): rank r owns grid r
+    from paper_2510_05282_b200 import inputs as _inputs
+
+    lo, hi = _inputs.shard_range(world * len(grid), rank, world)
+    assert hi - lo == len(grid) and lo % len(grid) == 0
+    pts = grid
     n = len(pts)
     nrep_in, nrep_out = 4, 2  # 4 x 50 MB inputs > L2; outputs 1.68 GB each
     xs = [torch.from_numpy(pts).to(dev) for _ in range(nrep_in)]
@@ -465,11 +601,14 @@ def run_ours(args):
     e2e_s = max_over_ranks(e2e_s, dev)
     # spot-check the end-to-end result against the device-resident result
     assert torch.equal(h_aos[:1000], out_aos[(args.steps - 1) % nrep_out][:1000].cpu())
+    assert torch.equal(h_soa[:, :1000], out_soa[(args.steps - 1) % nrep_out][:, :1000].cpu())
 
     if rank == 0:
         peak, peak_src = measured_peak()
+        del out_soa, out_aos, xs
+        torch.cuda.empty_cache()
+        ceil = ceilings(dev, local) if (world == 1 and not args.no_ceilings) else None
         dom = ("sh_real lmax=9 SoA", t_soa, "soa") if t_soa >= t_aos else ("sh_real lmax=9 AoS", t_aos, "aos")
-        achieved = BYTES_PER_POINT * n / (dom[1] * 1e-3) / 1e9
         values_per_step = 2 * n * K
         line = {
             "metric": METRIC, "value": world * args.steps * values_per_step / (ms * 1e-3) / 1e9, "unit": UNIT,
@@ -481,24 +620,24 @@ def run_ours(args):
             "gpu_launches": int(launches),
             "clocks": clocks,
             "kernels": {
-                "sh_real_soa": {"ms": t_soa, "write_GBps": 8 * K * n / (t_soa * 1e-3) / 1e9, "G_values_per_s": n * K / (t_soa * 1e-3) / 1e9},
-                "sh_real_aos": {"ms": t_aos, "write_GBps": 8 * K * n / (t_aos * 1e-3) / 1e9, "G_values_per_s": n * K / (t_aos * 1e-3) / 1e9},
+                "sh_real_soa": {"ms": t_soa, "write_GBps": 8 * K * n / (t_soa * 1e-3) / 1e9, "G_values_per_s": n * K / (t_soa * 1e-3) / 1e9,
+                                "roofline": hbm_roofline("sh_real lmax=9 SoA", BYTES_PER_POINT * n, 8 * K * n, t_soa, peak, peak_src, ceil, "soa_planes", "real_soa")},
+                "sh_real_aos": {"ms": t_aos, "write_GBps": 8 * K * n / (t_aos * 1e-3) / 1e9, "G_values_per_s": n * K / (t_aos * 1e-3) / 1e9,
+                                "roofline": hbm_roofline("sh_real lmax=9 AoS", BYTES_PER_POINT * n, 8 * K * n, t_aos, peak, peak_src, ceil, "bulk_tiles", "real_aos")},
             },
-            "roofline": {
-                "bound": "hbm", "kernel": dom[0], "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "peak_source": peak_src, "algorithmic_bytes_per_launch": BYTES_PER_POINT * n, "avg_launch_ms": dom[1],
-                "traffic": ncu_traffic(dom[2]),
-            },
+            "roofline": hbm_roofline(dom[0], BYTES_PER_POINT * n, 8 * K * n, dom[1], peak, peak_src, ceil,
+                                     "soa_planes" if dom[2] == "soa" else "bulk_tiles", traffic_key="real_" + dom[2]),
             "e2e": {"value": world * e2e_steps * values_per_step / e2e_s / 1e9, "unit": UNIT,
                     "h2d_bytes_per_step": 2 * n * 24, "d2h_bytes_per_step": 2 * n * K * 8, "steps": e2e_steps,
                     "api": "sh_real_host (pinned host buffers)"},
         }
+        if ceil:
+            line["ceilings"] = ceil
         if world == 1 and not args.no_extras:
-            del out_soa, out_aos, xs
-            torch.cuda.empty_cache()
-            line["other_configs"] = extra_configs(sh, dev, args.only)
+            line["other_configs"] = extra_configs(sh, dev, args.only, ceil)
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(pts)
+            line["cpu_method"] = cpu_method(pts)
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -512,6 +651,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the untimed-by-`value` runs of the other configs")
+    ap.add_argument("--no-ceilings", action="store_true", help="skip the write-fill / DFMA ceiling measurements (csrc/sh_peaks.cu)")
     ap.add_argument("--tune", action="append", default=[], metavar="KNOB=VALUE",
                     help="override a launch heuristic for the whole run (binding.TUNE names, e.g. soa_split=2); recorded in config")
     ap.add_argument("--only", default=None, help="run only the other-config cases whose name contains this substring")

@@ -23,8 +23,12 @@
  *
  * Pointers: every `xyz` / `out` of the sh_real / sh_complex / sh_spinor / sh_real_f32 calls is a DEVICE
  * pointer (global memory of the current CUDA device); `xyz` is AoS [n][3].  The *_host calls take HOST
- * pointers.  The caller owns all buffers; the library allocates nothing on the device calls, keeps no
- * state between calls and is re-entrant.  Device calls are asynchronous: they enqueue kernels on
+ * pointers.  The caller owns all buffers; the device calls allocate nothing and may be issued concurrently from several
+ * threads and on several devices.  What the library does keep, process-wide: the sh_set_tuning() knobs (benchmarking only;
+ * they select among kernels with identical results, so a concurrent caller can see another kernel but never another value),
+ * per-device caches of pure device properties (SM count, granted shared-memory opt-ins), a launch counter, the last CUDA
+ * error text (per thread), and the staging pool of the *_host calls (created on first use, serialised by a mutex, freed by
+ * sh_host_release()).  Device calls are asynchronous: they enqueue kernels on
  * `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream) and return without
  * synchronizing.  `out` must be aligned to its element type (8 B for sh_real, 4 B for sh_real_f32); 16-byte
  * aligned `out` (and, for SoA, even n) enables the vectorised / bulk-copy store paths, anything else falls
@@ -162,19 +166,18 @@ int sh_index_real(int l, int m);
  * -1 if the triple is not a valid spin-1/2 state with l <= 9. */
 int sh_index_spinor(int l, int twoj, int twomj);
 
-/* Launch-heuristic overrides, for benchmarking and tuning only: process-global, do not change results.
- * value 0 restores the built-in default; returns SH_ERR_LAYOUT for an unknown knob or a negative value. */
+/* Launch-heuristic overrides, for benchmarking and A/B measurements only: process-global, do not change results (every
+ * value selects among kernels that compute the same arithmetic).  value 0 restores the built-in default; returns
+ * SH_ERR_LAYOUT for an unknown knob or a negative value. */
 enum {
-    SH_TUNE_SOA_TILES_PER_CTA = 0,  /* consecutive 256-point tiles one CTA of the SoA kernels processes */
-    SH_TUNE_AOS_TILES_PER_WARP = 1, /* consecutive 32-point tiles one warp of the AoS kernels processes */
-    SH_TUNE_PREFETCH_WINDOW_POINTS = 2, /* points per burst of the L2 input prefetch (default 262144); 1 = prefetch off */
-    SH_TUNE_PROJ_AOS_MODE = 3,      /* sh_projectors AoS copy-out: 1 = warp copy, 2 = one bulk copy per row, 3 = one per tile (when possible) */
-    SH_TUNE_SOA_TMA = 4,            /* sh_real / sh_real_f32 SoA through one TMA tensor store per tile of 1 KB rows (128 / 256 points): 0 = when possible (default), 1 = never */
-    SH_TUNE_PROJECT_FORM = 5,       /* sh_project polynomials: 0 = the factorized forms of every other call (default); 1 = Horner in z^2 for the
-                                       polar factors and (x + iy)^m by recurrence: ~35 % fewer FP64 instructions, same tolerance */
-    SH_TUNE_PROJ_AOS_SPLIT = 6,     /* sh_projectors AoS, lmax >= 4: warps that share one 32-point tile, each evaluating part of the l-blocks: 1, 2 (default) or 4 */
-    SH_TUNE_SOA_SPLIT = 7,          /* sh_real / sh_real_f32 SoA tensor-store path, lmax >= 4: warps that share a 32-point group of the tile, each evaluating part of the l-blocks: 1 or 2 (default) */
-    SH_TUNE_COUNT = 8
+    SH_TUNE_PREFETCH_WINDOW_POINTS = 0, /* points per burst of the L2 input prefetch (default 262144); 1 = prefetch off */
+    SH_TUNE_PROJ_AOS_MODE = 1,      /* sh_projectors AoS copy-out: 1 = warp copy, 2 = one bulk copy per row, 3 = one per tile (when possible) */
+    SH_TUNE_SOA_TMA = 2,            /* SoA through TMA tensor stores (tiles staged in shared memory): 0 = when possible (default), 1 = never (per-thread streaming stores) */
+    SH_TUNE_PROJECT_FORM = 3,       /* sh_project polynomials: 0 = default; 1 = Horner in z^2 for the polar factors and (x + iy)^m by
+                                       recurrence; 2 = the factorized root-pair forms of every other call */
+    SH_TUNE_PROJ_AOS_SPLIT = 4,     /* sh_projectors AoS, lmax >= 4: warps that share one 32-point tile, each evaluating part of the l-blocks: 1, 2 (default) or 4 */
+    SH_TUNE_SOA_SPLIT = 5,          /* sh_real / sh_real_f32 SoA tensor-store path, lmax >= 4: warps that share a 32-point group of the tile, each evaluating part of the l-blocks: 1 or 2 (default) */
+    SH_TUNE_COUNT = 6
 };
 int sh_set_tuning(int knob, int value);
 

@@ -111,7 +111,7 @@ def index_spinor(l: int, twoj: int, twomj: int) -> int:
     return load().sh_index_spinor(l, twoj, twomj)
 
 
-TUNE = {"soa_tiles_per_cta": 0, "aos_tiles_per_warp": 1, "prefetch_window_points": 2, "proj_aos_mode": 3, "soa_tma": 4, "project_form": 5, "proj_aos_split": 6, "soa_split": 7}
+TUNE = {"prefetch_window_points": 0, "proj_aos_mode": 1, "soa_tma": 2, "project_form": 3, "proj_aos_split": 4, "soa_split": 5}
 
 
 def set_tuning(knob, value: int) -> None:
@@ -195,27 +195,51 @@ def sh_complex_ext(xyz, lmax, out=None, layout="soa", store="auto", stream=None,
     return _device_call("complex_ext", xyz, lmax, out, layout, store, stream, coords)
 
 
-def host_call(kind: str, xyz: "np.ndarray | object", lmax: int, out=None, layout="soa", coords="cartesian"):
-    """sh_*_host: HOST buffers in and out (numpy arrays or CPU torch tensors, ideally pinned)."""
+def host_call(kind: str, xyz, lmax: int, out=None, layout="soa", coords="cartesian"):
+    """sh_*_host: HOST buffers in and out (numpy arrays or CPU torch tensors, ideally pinned).  `xyz` may be anything numpy
+    can convert (it is copied if it is not a C-contiguous array of the right dtype); `out`, when given, is written in
+    place and must therefore already be a C-contiguous array / CPU tensor of the right dtype and size."""
     fn = getattr(load(), f"sh_{kind}_host")
     dt = np.float32 if kind == "real_f32" else np.float64
+    width = 2 if coords == "angular" else 3
 
-    def ptr_n(a):
-        if hasattr(a, "data_ptr"):
-            return a.data_ptr(), a
-        a = np.ascontiguousarray(a, dtype=dt)
-        return a.ctypes.data, a
+    def is_tensor(a):
+        return hasattr(a, "data_ptr")
 
-    xp, xk = ptr_n(xyz)
+    def check_tensor(a, what):
+        import torch
+
+        want = torch.float32 if kind == "real_f32" else torch.float64
+        if a.is_cuda or a.dtype != want or not a.is_contiguous():
+            raise ValueError(f"{what} must be a contiguous CPU tensor of {want}")
+
+    if is_tensor(xyz):
+        check_tensor(xyz, "xyz")
+        if xyz.dim() != 2 or xyz.shape[1] != width:
+            raise ValueError(f"xyz must be [n][{width}]")
+        xp, xk = xyz.data_ptr(), xyz
+    else:
+        xk = np.ascontiguousarray(xyz, dtype=dt)
+        if xk.ndim != 2 or xk.shape[1] != width:
+            raise ValueError(f"xyz must be [n][{width}]")
+        xp = xk.ctypes.data
     n = xk.shape[0]
     shape = out_shape(kind, n, lmax, layout)
     if out is None:
         out = np.empty(shape, dtype=dt)
-    op, ok = ptr_n(out)
+    if is_tensor(out):
+        check_tensor(out, "out")
+        if out.numel() != math.prod(shape):
+            raise ValueError(f"out must hold {math.prod(shape)} elements")
+        op = out.data_ptr()
+    else:
+        if not (isinstance(out, np.ndarray) and out.dtype == dt and out.flags.c_contiguous and out.flags.writeable and out.size == math.prod(shape)):
+            raise ValueError(f"out must be a writeable C-contiguous numpy array of {np.dtype(dt)} with {math.prod(shape)} elements")
+        op = out.ctypes.data
     rc = fn(xp, n, int(lmax), op, _LAYOUTS[layout] | _COORDS[coords])
     if rc != 0:
         raise ShError(rc, f"sh_{kind}_host")
-    return ok
+    return out
 
 
 # ---- fused projector consumer (include/shb200.h "Fused projector consumer") ----

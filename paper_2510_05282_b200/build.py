@@ -14,6 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libshb200.so")
+PEAKS_LIB = os.path.join(HERE, "libshb200_peaks.so")   # ceilings microbenchmarks (csrc/sh_peaks.cu): bench.py only, never linked into LIB
 # one harmonic kind per unit (they compile in parallel), the l > 9 extension, the fused projector consumer, shared host state
 SOURCES = ["sh_real.cu", "sh_complex.cu", "sh_spinor.cu", "sh_real_f32.cu", "sh_ext.cu", "sh_projector.cu", "sh_abi.cu"]
 HEADERS = ["sh_core.cuh", "sh_store.cuh", "sh_generated.cuh"]
@@ -60,6 +61,7 @@ def build(force: bool = False, verbose: bool = False, extra_flags: tuple = ()) -
         raise RuntimeError("nvcc failed for " + ", ".join(failed))
     with open(stamp, "w") as f:
         f.write(" ".join(flags))
+    build_peaks()
     objs = [os.path.join(objdir, s[:-3] + ".o") for s in SOURCES]
     if not jobs and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(o) for o in objs):
         return LIB
@@ -69,12 +71,24 @@ def build(force: bool = False, verbose: bool = False, extra_flags: tuple = ()) -
     return LIB
 
 
+def build_peaks(force: bool = False) -> str:
+    """csrc/sh_peaks.cu -> libshb200_peaks.so: the write-only fill and DFMA ceilings bench.py measures in the same run."""
+    src = os.path.join(CSRC, "sh_peaks.cu")
+    if force or not os.path.exists(PEAKS_LIB) or os.path.getmtime(PEAKS_LIB) < os.path.getmtime(src):
+        tmp = PEAKS_LIB + f".tmp{os.getpid()}"
+        subprocess.check_call([_nvcc()] + NVCC_FLAGS + ["-shared", "-o", tmp, src])
+        os.replace(tmp, PEAKS_LIB)
+    return PEAKS_LIB
+
+
 def ensure_built() -> str:
     """Compile only if libshb200.so is absent (a fresh checkout on a box that has nvcc).  Never a fallback: the result is
     the same CUDA library, and binding.load() still raises if it cannot be produced."""
+    if not os.path.exists(PEAKS_LIB):
+        build_peaks()
     return LIB if os.path.exists(LIB) else build(force=True)
 
 
 if __name__ == "__main__":
-    # extra nvcc flags (e.g. -DSHB200_DEV_ONLY_LMAX9 for development builds) pass through
+    # extra nvcc -D flags pass through
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, extra_flags=tuple(a for a in sys.argv[1:] if a.startswith("-D"))))

@@ -13,16 +13,15 @@ int cuda_fail(cudaError_t e) {
     return SH_ERR_CUDA;
 }
 
+// SMs of the CURRENT device (cached per device; 148 on a B200)
 int sm_count() {
-    static int sms = 0;
-    if (!sms) {
+    static PerDeviceInt cache;
+    const int sms = cache.get([] {
         int dev = 0, v = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0)
-            sms = v;
-        else
-            return 148;
-    }
-    return sms;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) return v;
+        return 0;
+    });
+    return sms > 0 ? sms : 148;
 }
 
 // launch-heuristic overrides (sh_set_tuning); 0 = default

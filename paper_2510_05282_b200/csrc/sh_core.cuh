@@ -365,23 +365,16 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)_
 
 // TMA bulk store shared -> global (cp.async.bulk, one bulk group per call site's commit).  The output is never re-read,
 // so its lines carry the L2 evict-first policy, like the st.global.cs of the LSU store paths: they leave L2 ahead of the
-// evict-last input prefetch and in the order they were written (SHB200_BULK_HINT = 0: no hint; measured in DESIGN.md section 6).
-#ifndef SHB200_BULK_HINT
-#define SHB200_BULK_HINT 1
-#endif
+// evict-last input prefetch and in the order they were written (without the hint: +1-3 % time).
 __device__ __forceinline__ uint64_t l2_evict_first_policy() {
     uint64_t pol;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     return pol;
 }
 __device__ __forceinline__ void bulk_store(void* gdst, const void* ssrc, int bytes) {
-#if SHB200_BULK_HINT
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes),
                  "l"(l2_evict_first_policy())
                  : "memory");
-#else
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes) : "memory");
-#endif
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -399,6 +392,22 @@ inline int launch_status() {
     const cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? SH_OK : cuda_fail(e);
 }
+
+// A small per-device cache of a pure function of (kernel, device): 0 = not computed yet.  Racing threads compute the same value.
+struct PerDeviceInt {
+    std::atomic<int> v[64];   // static storage: zero-initialised
+    template <class F> int get(F&& compute) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return compute();
+        std::atomic<int>& slot = v[dev & 63];
+        int x = slot.load(std::memory_order_relaxed);
+        if (x <= 0) {
+            x = compute();
+            if (x > 0) slot.store(x, std::memory_order_relaxed);
+        }
+        return x;
+    }
+};
 
 // Dynamic shared memory above 48 KB is an opt-in per kernel AND per device (cudaFuncSetAttribute acts on the current device):
 // the largest size granted so far is remembered per device, so a process that drives several GPUs opts in on each.
@@ -429,12 +438,7 @@ EncodeTiledFn encode_tiled();
 // four CTAs per SM, i.e. whole rows of a 32-point tile staged densely in <= 55 KB (complex lmax = 9: 51.2 KB), and
 // staging stores that conflict at most 4-way: 16-byte stores of a quarter warp land gcd(row_bytes/16, 8) deep; rows that
 // are not multiples of 16 B are staged with scalar stores, conflict-free because the row is then an odd number of words
-#ifndef SHB200_TILEBULK_WARPS
-#define SHB200_TILEBULK_WARPS 1
-#endif
-#ifndef SHB200_TILEBULK_MAX_CONFLICT
-#define SHB200_TILEBULK_MAX_CONFLICT 4
-#endif
-constexpr int TILEBULK_WARPS = SHB200_TILEBULK_WARPS;
+constexpr int TILEBULK_WARPS = 1;
+constexpr int TILEBULK_MAX_CONFLICT = 4;
 
 }  // namespace shb200

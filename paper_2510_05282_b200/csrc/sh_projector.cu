@@ -211,13 +211,7 @@ __global__ void __launch_bounds__(32 * SPLIT) sh_proj_aos_kernel(const double* _
 // Running sums are kept in the order of production ("slot order"); at the end a CTA adds its four warps in a fixed order
 // and writes one row of `partial` [cta][nvec][ncols]; sh_project_reduce_kernel adds the rows in a fixed order and
 // scatters to the caller's column order.
-#ifndef SHB200_PROJ_CTAS_NV1
-#define SHB200_PROJ_CTAS_NV1 4
-#endif
-#ifndef SHB200_PROJ_CTAS_NV4
-#define SHB200_PROJ_CTAS_NV4 3
-#endif
-constexpr int PROJ_CTAS_NV1 = SHB200_PROJ_CTAS_NV1, PROJ_CTAS_NV4 = SHB200_PROJ_CTAS_NV4;   // resident CTAs per SM (__launch_bounds__): register budget
+constexpr int PROJ_CTAS_NV1 = 4, PROJ_CTAS_NV4 = 3;   // resident CTAs per SM (__launch_bounds__): register budget
 constexpr int PROJ_NV = 4;          // weight vectors contracted per launch
 constexpr int PROJ_MAX_COLS = 128;  // columns per launch (whole channels); wider channel lists run as several launches
 constexpr int PROJ_SEG_PITCH = 34;  // doubles between consecutive columns of the transposed segment tile
@@ -440,9 +434,7 @@ int check_projector_args(const double* xyz, int64_t n, int nproj, const int* pro
 constexpr int PROJ_CTAS_PER_SM = PROJ_CTAS_NV1 > PROJ_CTAS_NV4 ? PROJ_CTAS_NV1 : PROJ_CTAS_NV4;   // grid cap of sh_project_kernel: the machine filled once (what the workspace is sized for)
 
 // warps per tile (block_part): the default comes from the 128^3-grid measurements in DESIGN.md section 6
-#ifndef SHB200_PROJ_AOS_SPLIT
-#define SHB200_PROJ_AOS_SPLIT 2
-#endif
+constexpr int PROJ_AOS_SPLIT = 2;
 
 template <int LMAX, int SPLIT>
 int launch_proj_aos_split(const double* xyz, int64_t n, const double* radial, const ProjPlan& plan, double* out, int pitch, int mode, size_t smem,
@@ -476,7 +468,7 @@ int launch_proj_aos(const double* xyz, int64_t n, const double* radial, const Pr
     const size_t smem = (size_t)32 * (pitch + plan.first[shgen::LMAX_CAP + 1]) * sizeof(double);   // row tile + radial values
     if (smem > (size_t)227 * 1024) return SH_ERR_PROJECTOR;
     // warps per tile: splitting pays once there are several l-blocks to share
-    int split = LMAX >= 4 ? tuned(SH_TUNE_PROJ_AOS_SPLIT, SHB200_PROJ_AOS_SPLIT) : 1;
+    int split = LMAX >= 4 ? tuned(SH_TUNE_PROJ_AOS_SPLIT, PROJ_AOS_SPLIT) : 1;
     if constexpr (LMAX >= 4) {
         if (split >= 4) return launch_proj_aos_split<LMAX, 4>(xyz, n, radial, plan, out, pitch, mode, smem, st);
         if (split >= 2) return launch_proj_aos_split<LMAX, 2>(xyz, n, radial, plan, out, pitch, mode, smem, st);
@@ -507,10 +499,7 @@ int run_projectors(const double* xyz, int64_t n, int nproj, const int* proj_l, c
     switch (lmax) {
 #define SH_CASE(L) case L: return layout_bits == SH_LAYOUT_SOA ? launch_proj_soa<L>(xyz, n, radial, plan, out, st) \
                                                              : launch_proj_aos<L>(xyz, n, radial, plan, out, st);
-#ifndef SHB200_DEV_ONLY_LMAX9
-        SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8)
-#endif
-        SH_CASE(3) SH_CASE(9)
+        SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(3) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8) SH_CASE(9)
 #undef SH_CASE
     }
     return SH_ERR_PROJECTOR;
@@ -550,7 +539,7 @@ int launch_project(const double* xyz, int64_t n, const double* radial, const Pro
     // per warp: segment tile, running sums, (weights,) and the radial values of every slot: 38 / 54 KB + 1 KB per slot per CTA
     const size_t slots_bytes = (size_t)4 * 32 * plan.first[shgen::LMAX_CAP + 1] * sizeof(double);
     constexpr size_t smem_max = (size_t)4 * (project_smem_doubles_per_warp<PROJ_NV>() + 32 * SH_MAX_PROJ) * sizeof(double);   // 86 KB
-    const bool fast = tuned(SH_TUNE_PROJECT_FORM, 0) == 1;   // Horner / recurrence forms instead of the factorized ones
+    const bool fast = tuned(SH_TUNE_PROJECT_FORM, 1) != 2;   // Horner / recurrence forms (default) or the factorized ones (knob value 2)
     auto launch = [&](auto kern, size_t warp_doubles, SmemOptIn& opted_in) -> int {
         if (const int rc = ensure_dynamic_smem(kern, smem_max, opted_in); rc != SH_OK) return rc;
         kern<<<(unsigned)blocks, 128, (size_t)4 * warp_doubles * sizeof(double) + slots_bytes, st>>>(xyz, n, radial, plan, seg, w, nvec, partial);
@@ -604,10 +593,7 @@ int run_project(const double* xyz, int64_t n, int nproj, const int* proj_l, cons
             const int nv = nvec - v0 < PROJ_NV ? nvec - v0 : PROJ_NV;
             switch (lmax) {
 #define SH_CASE(L) case L: rc = launch_project<L>(xyz, n, radial, plan, seg, w + (int64_t)v0 * n, nv, partial, coeff + (int64_t)v0 * ncols + c0, ncols, st); break;
-#ifndef SHB200_DEV_ONLY_LMAX9
-                SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8)
-#endif
-                SH_CASE(3) SH_CASE(9)
+                SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(3) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8) SH_CASE(9)
 #undef SH_CASE
             }
             if (rc != SH_OK) return rc;

@@ -35,49 +35,34 @@ struct SoASink {
     template <int L> __device__ __forceinline__ void polar(const T (&)[L + 1]) {}
 };
 
+// One 256-point tile per CTA: with the burst L2 prefetch the input load is an L2 hit, and a deep grid lets the hardware CTA
+// scheduler balance the SMs (251 vs 256 / 258 us for 1 / 2 / 4 tiles per CTA on the 128^3 grid at lmax = 9).
 template <int KIND, int LMAX, typename T, typename TI, int VEC, bool ANGULAR>
-__global__ void __launch_bounds__(256) sh_soa_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out, int tiles_per_cta, int coords, InputPrefetch pf) {
+__global__ void __launch_bounds__(256) sh_soa_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out, int coords, InputPrefetch pf) {
     constexpr int ES = elem_scalars(KIND);
     constexpr int IN_BYTES = (ANGULAR ? 2 : 3) * sizeof(TI);
-    prefetch_input_window(xyz, n * IN_BYTES, (int64_t)tiles_per_cta * 256 * IN_BYTES, pf);
-    const int64_t ntiles = (n + 255) >> 8;
-    int64_t t = (int64_t)blockIdx.x * tiles_per_cta;
-    const int64_t tend = (t + tiles_per_cta < ntiles) ? t + tiles_per_cta : ntiles;
-    int64_t i = (t << 8) + threadIdx.x;
-    RawPoint<TI, ANGULAR> cur, nxt;
-    bool have = i < n;
-    if (have) cur.load(xyz, i);
-    for (; t < tend; ++t, i += 256) {
-        const bool have_next = (t + 1 < tend) && (i + 256 < n);
-        if (have_next) nxt.load(xyz, i + 256);
-        if (have) {
-            SoASink<T, VEC> sink{out + i * ES, n * ES};
-            evaluate<KIND, LMAX, T>(cur.unit(coords), sink);
-        }
-        cur = nxt;
-        have = have_next;
-    }
+    prefetch_input_window(xyz, n * IN_BYTES, (int64_t)256 * IN_BYTES, pf);
+    const int64_t i = ((int64_t)blockIdx.x << 8) + threadIdx.x;
+    if (i >= n) return;
+    RawPoint<TI, ANGULAR> pt;
+    pt.load(xyz, i);
+    SoASink<T, VEC> sink{out + i * ES, n * ES};
+    evaluate<KIND, LMAX, T>(pt.unit(coords), sink);
 }
 
-// a8, SoA through the TMA tensor unit (real fp64).  One warp = one 32-point tile; lane i stages value k of its point at
-// tile[k][i] (8-byte stores, 32 consecutive doubles per plane: conflict-free), and after a proxy fence lane 0 issues ONE
-// cp.async.bulk.tensor.2d store of the box {32 points, K planes} through a tensor map of `out` viewed as [K][n]: K rows of
-// 256 contiguous bytes, each two full 128-byte lines.  The LSU issues no global store at all (100 STG + their address
-// arithmetic per point in sh_soa_kernel), and points past n in a ragged last tile are clipped by the tensor unit.
-// One warp per CTA for the same reason as the AoS tile-bulk path (fence.proxy.async is CTA-scoped).
-#ifndef SHB200_SOA_TMA_WARPS
-#define SHB200_SOA_TMA_WARPS 4
-#endif
-// warps per CTA = 32-point groups per tile.  Longer rows are what the tile buys: 258 / 258 / 250 / 345 us for 1 / 2 / 4 / 8 warps
-// (rows of 256 B .. 2 KB; 8 warps = one 205 KB tile per SM, nothing overlaps) on the 128^3 grid at lmax = 9.
-// (The fp32 variant gains nothing from it -- 255 vs 257 us on 2^22 points -- and stays on sh_soa_pair_kernel.)
-constexpr int SOA_TMA_WARPS = SHB200_SOA_TMA_WARPS;
-// warps sharing a 32-point group (lmax >= 4): 1 or 2.  Two warps, each evaluating part of the l-blocks, shorten a tile's
+// a8, SoA through the TMA tensor unit (sh_real fp64 and sh_real_f32).  One CTA = one tile of PTS points = SOA_TMA_WARPS groups
+// of 32 points; thread i stages value k of its point at tile[k][i] (conflict-free 8-byte / 4-byte shared stores: consecutive
+// lanes, consecutive words), and after a proxy fence and a CTA barrier thread 0 issues ONE cp.async.bulk.tensor.2d store of
+// the box {PTS points, K planes} through a tensor map of `out` viewed as [K][n]: K rows of 1 KB (128 fp64 / 256 fp32 points).
+// The LSU issues no global store at all (100 STG + their address arithmetic per point in sh_soa_kernel), and points past n
+// in a ragged last tile are clipped by the tensor unit.
+// Groups per tile: longer rows are what the tile buys -- 258 / 258 / 250 / 345 us for 1 / 2 / 4 / 8 groups (rows of
+// 256 B .. 2 KB; 8 groups = one 205 KB tile per SM, nothing overlaps) on the 128^3 grid at lmax = 9.
+constexpr int SOA_TMA_WARPS = 4;
+// Warps sharing a 32-point group (lmax >= 4): two warps, each evaluating part of the l-blocks (block_part), shorten a tile's
 // compute phase, so the two resident CTAs overlap their tensor stores better: 0.2499 -> 0.2477 ms on the 128^3 grid at
-// lmax = 9 (with 64-point tiles the split changes nothing: 0.2585 ms either way -- row length, not compute, bounds those)
-#ifndef SHB200_SOA_SPLIT
-#define SHB200_SOA_SPLIT 2
-#endif
+// lmax = 9 (with 64-point tiles the split changes nothing: 0.2585 ms either way -- row length, not compute, bounds those).
+constexpr int SOA_SPLIT = 2;
 
 template <int PTS, typename T = double>
 struct TileSink {
@@ -121,15 +106,9 @@ __global__ void __launch_bounds__(32 * WARPS * SPLIT, sizeof(T) == 4 ? 2 : 0) sh
     if constexpr (WARPS * SPLIT == 1) __syncwarp();
     else __syncthreads();
     if (threadIdx.x == 0) {
-#if SHB200_BULK_HINT
         asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%1, %2}], [%3], %4;" ::"l"(&tmap), "r"((int)base), "r"(0),
                      "r"(smem_u32(tile)), "l"(l2_evict_first_policy())
                      : "memory");
-#else
-        asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];" ::"l"(&tmap), "r"((int)base), "r"(0),
-                     "r"(smem_u32(tile))
-                     : "memory");
-#endif
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory is released when the CTA exits
     }
@@ -146,34 +125,18 @@ struct SoAPairSink {
 };
 
 template <int LMAX>
-__global__ void __launch_bounds__(256) sh_soa_pair_kernel(const float* __restrict__ xyz, int64_t n, float* __restrict__ out, int tiles_per_cta, int coords, InputPrefetch pf) {
-    prefetch_input_window(xyz, n * 12, (int64_t)tiles_per_cta * 512 * 12, pf);
-    const int64_t npairs = n >> 1;
-    const int64_t ntiles = (npairs + 255) >> 8;
-    int64_t t = (int64_t)blockIdx.x * tiles_per_cta;
-    const int64_t tend = (t + tiles_per_cta < ntiles) ? t + tiles_per_cta : ntiles;
-    int64_t j = (t << 8) + threadIdx.x;
-    auto load6 = [&](int64_t jj, float2& a, float2& b, float2& c) {
-        const float2* q = reinterpret_cast<const float2*>(xyz + 6 * jj);   // 24 B per pair: three 8-byte loads
-        a = __ldg(q); b = __ldg(q + 1); c = __ldg(q + 2);
-    };
-    float2 ca, cb, cc, na, nb, nc;
-    bool have = j < npairs;
-    if (have) load6(j, ca, cb, cc);
-    for (; t < tend; ++t, j += 256) {
-        const bool have_next = (t + 1 < tend) && (j + 256 < npairs);
-        if (have_next) load6(j + 256, na, nb, nc);
-        if (have) {
-            SoAPairSink sink{out + 2 * j, n};
-            // one copy of the polynomial code: only the front end branches (straight-line code size is instruction-fetch traffic)
-            UnitVec u0, u1;
-            if (coords == SH_COORDS_CARTESIAN) { u0 = normalize(ca.x, ca.y, cb.x); u1 = normalize(cb.y, cc.x, cc.y); }
-            else { u0 = as_given(ca.x, ca.y, cb.x); u1 = as_given(cb.y, cc.x, cc.y); }
-            evaluate_pair<LMAX>(u0, u1, sink);
-        }
-        ca = na; cb = nb; cc = nc;
-        have = have_next;
-    }
+__global__ void __launch_bounds__(256) sh_soa_pair_kernel(const float* __restrict__ xyz, int64_t n, float* __restrict__ out, int coords, InputPrefetch pf) {
+    prefetch_input_window(xyz, n * 12, (int64_t)512 * 12, pf);
+    const int64_t j = ((int64_t)blockIdx.x << 8) + threadIdx.x;   // pair index
+    if (j >= (n >> 1)) return;
+    const float2* q = reinterpret_cast<const float2*>(xyz + 6 * j);   // 24 B per pair: three 8-byte loads
+    const float2 ca = __ldg(q), cb = __ldg(q + 1), cc = __ldg(q + 2);
+    SoAPairSink sink{out + 2 * j, n};
+    // one copy of the polynomial code: only the front end branches (straight-line code size is instruction-fetch traffic)
+    UnitVec u0, u1;
+    if (coords == SH_COORDS_CARTESIAN) { u0 = normalize(ca.x, ca.y, cb.x); u1 = normalize(cb.y, cc.x, cc.y); }
+    else { u0 = as_given(ca.x, ca.y, cb.x); u1 = as_given(cb.y, cc.x, cc.y); }
+    evaluate_pair<LMAX>(u0, u1, sink);
 }
 
 
@@ -345,48 +308,38 @@ struct RowSink {
     }
 };
 
+// One 32-point tile per warp: measured fastest on every bulk path now that the input arrives by the burst L2 prefetch (real
+// tile-bulk 238 / 242 / 249 us, spinor row-bulk 1002 / 1028 / 1064 us for 1 / 2 / 4 tiles per warp).
 template <int KIND, int LMAX, typename T, typename TI, int CAP, int MODE, int WARPS, bool ANGULAR>
-__global__ void __launch_bounds__(WARPS * 32) sh_aos_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out, int tiles_per_warp, int coords, InputPrefetch pf) {
+__global__ void __launch_bounds__(WARPS * 32) sh_aos_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out, int coords, InputPrefetch pf) {
     using Sink = RowSink<KIND, LMAX, T, CAP, MODE>;
     constexpr int IN_BYTES = (ANGULAR ? 2 : 3) * sizeof(TI);
-    prefetch_input_window(xyz, n * IN_BYTES, (int64_t)tiles_per_warp * WARPS * 32 * IN_BYTES, pf);
+    prefetch_input_window(xyz, n * IN_BYTES, (int64_t)WARPS * 32 * IN_BYTES, pf);
     static_assert(Sink::Seg::valid(), "CAP too small for one l-block group");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     T* tile = reinterpret_cast<T*>(smem_raw) + (size_t)warp * 32 * Sink::PITCH;
-    const int64_t ntiles = (n + 31) >> 5;
-    // warp w of CTA b owns tiles [(b*WARPS + w) * tiles_per_warp, +tiles_per_warp): a contiguous span of `out`
-    int64_t t = ((int64_t)blockIdx.x * WARPS + warp) * tiles_per_warp;
-    const int64_t tend = (t + tiles_per_warp < ntiles) ? t + tiles_per_warp : ntiles;
+    const int64_t base = ((int64_t)blockIdx.x * WARPS + warp) << 5;   // first point of the warp's tile
+    if (base >= n) return;
+    int64_t i = base + lane;
     // plain / tile-bulk mode: every lane takes part in the warp-level copy-out, so idle lanes of the last tile evaluate a clamped point
-    auto point_of = [&](int64_t tt) {
-        const int64_t i = (tt << 5) + lane;
-        return (MODE != MODE_ROWBULK && i >= n) ? n - 1 : i;
-    };
-    RawPoint<TI, ANGULAR> cur, nxt;
-    bool have = t < tend && point_of(t) < n;
-    if (have) cur.load(xyz, point_of(t));
-    for (; t < tend; ++t) {
-        const bool have_next = (t + 1 < tend) && point_of(t + 1) < n;
-        if (have_next) nxt.load(xyz, point_of(t + 1));
-        if (have) {
-            const int64_t base = t << 5;
-            const int64_t left = n - base;
-            Sink sink;
-            sink.row = tile + lane * Sink::PITCH;
-            sink.tile = tile;
-            sink.gout = out;
-            sink.base = base;
-            sink.rows = left < 32 ? (int)left : 32;
-            sink.lane = lane;
-            sink.i = point_of(t);
-            sink.wait_reads();   // bulk mode: the previous tile's copy has finished reading this lane's row
-            evaluate<KIND, LMAX, T>(cur.unit(coords), sink);
-        }
-        cur = nxt;
-        have = have_next;
+    if (i >= n) {
+        if constexpr (MODE == MODE_ROWBULK) return;
+        i = n - 1;
     }
-    if constexpr (MODE != MODE_PLAIN) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    RawPoint<TI, ANGULAR> pt;
+    pt.load(xyz, i);
+    const int64_t left = n - base;
+    Sink sink;
+    sink.row = tile + lane * Sink::PITCH;
+    sink.tile = tile;
+    sink.gout = out;
+    sink.base = base;
+    sink.rows = left < 32 ? (int)left : 32;
+    sink.lane = lane;
+    sink.i = i;
+    evaluate<KIND, LMAX, T>(pt.unit(coords), sink);
+    if constexpr (MODE != MODE_PLAIN) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory is released when the CTA exits
 }
 
 
@@ -394,15 +347,9 @@ __global__ void __launch_bounds__(WARPS * 32) sh_aos_kernel(const TI* __restrict
 // launchers
 template <int KIND, int LMAX, typename T, typename TI, int VEC, bool ANGULAR = false>
 int launch_soa(const TI* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
-    const int64_t tiles = (n + 255) / 256;
-    // one 256-point tile per CTA: with the burst L2 prefetch the input load is an L2 hit, and a deep grid lets the
-    // hardware CTA scheduler balance the SMs (251 vs 256 / 258 us for 1 / 2 / 4 tiles on the 128^3 grid at lmax = 9).
-    // With more tiles per CTA the next tile's input is loaded before the current tile is evaluated.
-    int tpc = tuned(SH_TUNE_SOA_TILES_PER_CTA, 1);
-    while (tpc > 1 && tiles / tpc < (int64_t)sm_count() * 16) tpc >>= 1;
-    const int64_t blocks = (tiles + tpc - 1) / tpc;
+    const int64_t blocks = (n + 255) / 256;
     if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
-    sh_soa_kernel<KIND, LMAX, T, TI, VEC, ANGULAR><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, out, tpc, coords, prefetch_plan(n, (int64_t)tpc * 256));
+    sh_soa_kernel<KIND, LMAX, T, TI, VEC, ANGULAR><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, out, coords, prefetch_plan(n, 256));
     return launch_status();
 }
 
@@ -434,7 +381,7 @@ int launch_soa_tma(const T* xyz, int64_t n, T* out, int coords, cudaStream_t st)
     };
     static SmemOptIn opted_in[2];
     if constexpr (LMAX >= 4) {
-        if (tuned(SH_TUNE_SOA_SPLIT, SHB200_SOA_SPLIT) >= 2) return launch(sh_soa_tma_kernel<T, LMAX, TMA_WARPS, 2, ANGULAR>, 2, opted_in[1]);
+        if (tuned(SH_TUNE_SOA_SPLIT, SOA_SPLIT) >= 2) return launch(sh_soa_tma_kernel<T, LMAX, TMA_WARPS, 2, ANGULAR>, 2, opted_in[1]);
     }
     return launch(sh_soa_tma_kernel<T, LMAX, TMA_WARPS, 1, ANGULAR>, 1, opted_in[0]);
 }
@@ -453,7 +400,7 @@ constexpr bool tile_bulk_ok() {
     if (row_bytes % 16 != 0) return true;
     int chunks = row_bytes / 16, g = 8;
     while (chunks % g) g >>= 1;
-    return g <= SHB200_TILEBULK_MAX_CONFLICT;
+    return g <= TILEBULK_MAX_CONFLICT;
 }
 
 template <int KIND, int LMAX, typename T, typename TI, int MODE, bool ANGULAR = false>
@@ -466,33 +413,17 @@ int launch_aos(const TI* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
     auto kern = sh_aos_kernel<KIND, LMAX, T, TI, CAP, MODE, WARPS, ANGULAR>;
     static SmemOptIn opted_in;
     if (const int rc = ensure_dynamic_smem(kern, smem, opted_in); rc != SH_OK) return rc;
-    static int ctas_per_sm = 0;   // idempotent cache of a pure function of the kernel
-    if (!ctas_per_sm) {
-        int occ = 0;
-        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, WARPS * 32, smem);
-        if (e != cudaSuccess) return cuda_fail(e);
-        ctas_per_sm = occ > 0 ? occ : 1;
-    }
-    const int64_t ntiles = (n + 31) / 32;
-    // one tile per warp measured fastest on every bulk path now that the input arrives by the burst L2 prefetch
-    // (real tile-bulk 238 / 242 / 249 us, spinor row-bulk 1002 / 1028 / 1064 us for 1 / 2 / 4 tiles per warp); with more
-    // tiles per warp the next tile's input is loaded before the current tile is evaluated
-    int tpw = tuned(SH_TUNE_AOS_TILES_PER_WARP, 1);
-    while (tpw > 1 && ntiles / ((int64_t)WARPS * tpw) < (int64_t)sm_count() * ctas_per_sm * 4) tpw >>= 1;
-    const int64_t blocks = (ntiles + (int64_t)WARPS * tpw - 1) / ((int64_t)WARPS * tpw);
+    const int64_t blocks = ((n + 31) / 32 + WARPS - 1) / WARPS;
     if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
-    kern<<<(unsigned)blocks, WARPS * 32, smem, st>>>(xyz, n, out, tpw, coords, prefetch_plan(n, (int64_t)tpw * WARPS * 32));
+    kern<<<(unsigned)blocks, WARPS * 32, smem, st>>>(xyz, n, out, coords, prefetch_plan(n, (int64_t)WARPS * 32));
     return launch_status();
 }
 
 template <int LMAX>
 int launch_soa_pair(const float* xyz, int64_t n, float* out, int coords, cudaStream_t st) {
-    const int64_t tiles = ((n >> 1) + 255) / 256;
-    int tpc = tuned(SH_TUNE_SOA_TILES_PER_CTA, 1);
-    while (tpc > 1 && tiles / tpc < (int64_t)sm_count() * 16) tpc >>= 1;
-    const int64_t blocks = (tiles + tpc - 1) / tpc;
+    const int64_t blocks = ((n >> 1) + 255) / 256;
     if (blocks > 0x7fffffffLL) return SH_ERR_COUNT;
-    sh_soa_pair_kernel<LMAX><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, out, tpc, coords, prefetch_plan(n, (int64_t)tpc * 512));
+    sh_soa_pair_kernel<LMAX><<<(unsigned)blocks, 256, 0, st>>>(xyz, n, out, coords, prefetch_plan(n, 512));
     return launch_status();
 }
 
@@ -567,10 +498,7 @@ int run_device(const TI* xyz, int64_t n, int lmax, T* out, int layout_bits, void
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     switch (lmax) {
 #define SH_CASE(L) case L: return dispatch_lmax<KIND, L, T, TI>(xyz, n, out, layout, path, coords, st);
-#ifndef SHB200_DEV_ONLY_LMAX9   /* development builds may compile the lmax = 9 kernels only */
-        SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(3) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8)
-#endif
-        SH_CASE(9)
+        SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(3) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8) SH_CASE(9)
 #undef SH_CASE
     }
     return SH_ERR_LMAX;

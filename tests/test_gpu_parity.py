@@ -297,7 +297,7 @@ def test_config3_full_grid_every_point(sh, oracle_mod, layout, store):
     assert worst <= TOL64, worst
 
 
-# ----------------------------------------------------------------------------- configs 4 and 5: full size on the GPU, sampled + properties
+# ----------------------------------------------------------------------------- configs 4 and 5: full size, EVERY point
 def sample_indices(n, k, seed):
     rng = np.random.default_rng(seed)
     idx = np.concatenate([np.arange(64), np.arange(n - 64, n), rng.integers(0, n, k)])
@@ -312,71 +312,123 @@ def run_full(sh, kind, x, lmax, layout):
     return out
 
 
-@pytest.mark.parametrize("layout", ["soa", "aos"])
-def test_config4_complex_2pow24(sh, oracle_mod, layout):
+def write_report(name, text):
+    """Reports the GPU tests produce are tracked artefacts (profiles/); a copy goes to gpurun_out/, the one folder that
+    comes back from the GPU box."""
+    import os
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    for d in ("profiles", "gpurun_out"):
+        os.makedirs(os.path.join(root, d), exist_ok=True)
+        with open(os.path.join(root, d, name), "w") as f:
+            f.write(text)
+
+
+def every_point_parity(sh, oracle_mod, kind, pts, lmax, tol, slab, report, title):
+    """parity over ALL points of a config.  The kernels run at full size in both layouts (the launch
+    configuration bench.py times); the results come back in slabs, the oracle evaluates the same slab, and every scalar is
+    compared.  Keeps the max abs error with its (layout, point, l, element) location, a per-l max / mean table, and the
+    error over the near-pole points (sin(theta) < 1e-3), which the paper names as the worst ones."""
     import torch
+
+    n = len(pts)
+    base = "real" if kind == "real_f32" else kind
+    x = torch.from_numpy(pts).cuda()
+    p64 = pts.astype(np.float64)
+    k = (lmax + 1) ** 2
+    ne = 2 * k if base == "spinor" else k
+    l_of = np.floor(np.sqrt(np.arange(ne) / (2 if base == "spinor" else 1)) + 1e-9).astype(int)
+    starts = np.searchsorted(l_of, np.arange(lmax + 1))
+    sin_theta = np.hypot(p64[:, 0], p64[:, 1]) / np.maximum(np.linalg.norm(p64, axis=1), 1e-300)
+    near = sin_theta < 1e-3
+    lines = [f"# {title}", f"# command: python -m pytest tests/test_gpu_parity.py -m gpu -k {report.split('.')[0].replace('parity_', '')}",
+             f"# N = {n} points, every point and every scalar compared with the oracle (slabs of {slab} points); tolerance {tol:g}",
+             f"# near-pole points (sin(theta) < 1e-3): {int(near.sum())}, smallest sin(theta) = {sin_theta[sin_theta > 0].min():.3e}"]
+    outs = {layout: run_full(sh, kind, x, lmax, layout) for layout in ("soa", "aos")}
+    stats = {layout: {"max": np.zeros(lmax + 1), "sum": np.zeros(lmax + 1), "worst": (0.0, -1, -1), "near": 0.0} for layout in outs}
+    for lo in range(0, n, slab):
+        hi = min(n, lo + slab)
+        want = oracle_eval(oracle_mod, base, p64[lo:hi], lmax).reshape(hi - lo, ne, -1)
+        for layout, out in outs.items():
+            got = out[:, lo:hi] if layout == "soa" else out[lo:hi]
+            got = got.cpu().numpy().astype(np.float64, copy=False).reshape((ne, hi - lo, -1) if layout == "soa" else (hi - lo, ne, -1))
+            if layout == "soa":
+                got = np.moveaxis(got, 0, 1)
+            d = np.abs(got - want)
+            assert not np.isnan(d).any(), (layout, lo)
+            per_elem = d.max(axis=2)                      # [points][ne]
+            st = stats[layout]
+            st["max"] = np.maximum(st["max"], np.maximum.reduceat(per_elem.max(axis=0), starts))
+            st["sum"] += np.add.reduceat(d.sum(axis=(0, 2)), starts)
+            w = float(per_elem.max())
+            if w > st["worst"][0]:
+                i, e = np.unravel_index(int(per_elem.argmax()), per_elem.shape)
+                st["worst"] = (w, lo + int(i), int(e))
+            if near[lo:hi].any():
+                st["near"] = max(st["near"], float(per_elem[near[lo:hi]].max()))
+            del got, d, per_elem
+        del want
+    es = {"real": 1, "complex": 2, "spinor": 4}[base]
+    counts = np.diff(np.append(starts, ne)) * es * n
+    for layout, st in stats.items():
+        w, i, e = st["worst"]
+        lines.append(f"\n[{layout}] max abs error {w:.3e} at point {i} ({p64[i, 0]:.6g}, {p64[i, 1]:.6g}, {p64[i, 2]:.6g}), l = {l_of[e]}, element {e}; "
+                     f"max over the near-pole points {st['near']:.3e}")
+        lines.append("l  max|gpu-oracle|  mean|gpu-oracle|")
+        for l in range(lmax + 1):
+            lines.append(f"{l}  {st['max'][l]:.3e}  {st['sum'][l] / counts[l]:.3e}")
+    text = "\n".join(lines) + "\n"
+    print(text)
+    write_report(report, text)
+    for layout, st in stats.items():
+        assert st["worst"][0] <= tol, (layout, st["worst"])
+    return outs
+
+
+def test_config4_complex_2pow24_every_point(sh, oracle_mod):
     from paper_2510_05282_b200 import inputs
 
     pts = inputs.config4_sphere_directions()
-    n = len(pts)
-    assert n == 1 << 24
-    x = torch.from_numpy(pts).cuda()
-    out = run_full(sh, "complex", x, 9, layout)  # 26.8 GB
-    idx = sample_indices(n, 60000, 41)
-    tidx = torch.from_numpy(idx).cuda()
-    got = (out[:, tidx].permute(1, 0, 2) if layout == "soa" else out[tidx]).contiguous().cpu().numpy()
-    want = oracle_eval(oracle_mod, "complex", pts[idx], 9)
-    assert max_err(got, want) <= TOL64
-    # property at every point: sum_m |Y_l^m|^2 = (2l+1)/(4 pi)
-    worst = 0.0
-    for l in range(10):
-        sl = slice(l * l, (l + 1) ** 2)
-        blk = out[sl] if layout == "soa" else out[:, sl]
-        dens = (blk * blk).sum(dim=(0, 2)) if layout == "soa" else (blk * blk).sum(dim=(1, 2))
-        worst = max(worst, float((dens - (2 * l + 1) / (4 * np.pi)).abs().max()))
-        del blk, dens
-    assert worst <= 1e-13, worst
+    assert len(pts) == 1 << 24
+    outs = every_point_parity(sh, oracle_mod, "complex", pts, 9, TOL64, 1 << 18, "parity_config4_complex.txt",
+                              "config 4: sh_complex, lmax = 9, 2^24 directions x log-uniform radii (seed 1), fp64")   # 2 x 26.8 GB on the device
+    # and the addition theorem at every point: sum_m |Y_l^m|^2 = (2l+1)/(4 pi)
+    for layout, out in outs.items():
+        worst = 0.0
+        for l in range(10):
+            sl = slice(l * l, (l + 1) ** 2)
+            blk = out[sl] if layout == "soa" else out[:, sl]
+            dens = (blk * blk).sum(dim=(0, 2)) if layout == "soa" else (blk * blk).sum(dim=(1, 2))
+            worst = max(worst, float((dens - (2 * l + 1) / (4 * np.pi)).abs().max()))
+            del blk, dens
+        assert worst <= 1e-13, (layout, worst)
 
 
-@pytest.mark.parametrize("layout", ["soa", "aos"])
-def test_config5_spinor_2pow22(sh, oracle_mod, layout):
-    import torch
+def test_config5_spinor_2pow22_every_point(sh, oracle_mod):
     from paper_2510_05282_b200 import inputs
 
     pts = inputs.config5_ball()
-    n = len(pts)
-    assert n == 1 << 22
-    x = torch.from_numpy(pts).cuda()
-    out = run_full(sh, "spinor", x, 9, layout)  # 26.8 GB
-    idx = sample_indices(n, 30000, 51)
-    tidx = torch.from_numpy(idx).cuda()
-    got = (out[:, tidx].permute(1, 0, 2) if layout == "soa" else out[tidx]).contiguous().cpu().numpy()
-    assert max_err(got, oracle_eval(oracle_mod, "spinor", pts[idx], 9)) <= TOL64
-    # property at every point: sum over the 2(2l+1) states of a given l of S^dagger S = 2 (2l+1)/(4 pi)
-    worst = 0.0
-    for l in range(10):
-        sl = slice(2 * l * l, 2 * (l + 1) ** 2)
-        blk = out[sl] if layout == "soa" else out[:, sl]
-        dens = (blk * blk).sum(dim=(0, 2)) if layout == "soa" else (blk * blk).sum(dim=(1, 2))
-        worst = max(worst, float((dens - 2 * (2 * l + 1) / (4 * np.pi)).abs().max()))
-        del blk, dens
-    assert worst <= 1e-13, worst
+    assert len(pts) == 1 << 22
+    outs = every_point_parity(sh, oracle_mod, "spinor", pts, 9, TOL64, 1 << 16, "parity_config5_spinor.txt",
+                              "config 5: sh_spinor, lmax = 9, 2^22 points uniform in a ball of radius 5 (seed 5), fp64")   # 2 x 26.8 GB on the device
+    # and at every point: sum over the 2(2l+1) states of a given l of S^dagger S = 2 (2l+1)/(4 pi)
+    for layout, out in outs.items():
+        worst = 0.0
+        for l in range(10):
+            sl = slice(2 * l * l, 2 * (l + 1) ** 2)
+            blk = out[sl] if layout == "soa" else out[:, sl]
+            dens = (blk * blk).sum(dim=(0, 2)) if layout == "soa" else (blk * blk).sum(dim=(1, 2))
+            worst = max(worst, float((dens - 2 * (2 * l + 1) / (4 * np.pi)).abs().max()))
+            del blk, dens
+        assert worst <= 1e-13, (layout, worst)
 
 
-@pytest.mark.parametrize("layout", ["soa", "aos"])
-def test_config5_real_f32_variant(sh, oracle_mod, layout):
-    import torch
+def test_config5_real_f32_variant_every_point(sh, oracle_mod):
     from paper_2510_05282_b200 import inputs
 
-    pts32 = inputs.config5_ball().astype(np.float32)
-    n = len(pts32)
-    x = torch.from_numpy(pts32).cuda()
-    out = run_full(sh, "real_f32", x, 9, layout)
-    idx = sample_indices(n, 200000, 52)
-    tidx = torch.from_numpy(idx).cuda()
-    got = (out[:, tidx].t() if layout == "soa" else out[tidx]).contiguous().cpu().numpy().astype(np.float64)
-    want = oracle_mod.real(pts32[idx].astype(np.float64), 9)
-    assert max_err(got, want) <= TOL32
+    pts32 = inputs.config5_ball().astype(np.float32)   # the oracle evaluates at the fp32 inputs, converted exactly (reading #21)
+    every_point_parity(sh, oracle_mod, "real_f32", pts32, 9, TOL32, 1 << 18, "parity_config5_real_f32.txt",
+                       "config 5, fp32 variant: sh_real_f32, lmax = 9, the 2^22 ball points cast to fp32")
 
 
 # ----------------------------------------------------------------------------- host-buffer entry points
@@ -446,9 +498,8 @@ def test_accuracy_study_like_fig1(sh, oracle_mod):
         assert ds.max() <= 1e-12  # the fp64 library itself loses digits near the poles
     report = "\n".join(lines)
     print(report)
-    os.makedirs("gpurun_out", exist_ok=True)
-    with open(os.path.join("gpurun_out", "accuracy_study.txt"), "w") as f:
-        f.write(report + "\n")
+    write_report("accuracy_study_like_fig1.txt", "# accuracy study in the manner of the paper's Fig. 1 (P:126-136): 5180 random points in a sphere, real harmonics, lmax = 9\n"
+                 "# command: python -m pytest tests/test_gpu_parity.py -m gpu -k accuracy_study\n" + report + "\n")
 
 
 # ----------------------------------------------------------------------------- l > 9 by recurrence
@@ -514,6 +565,35 @@ def test_ext_full_size_sampled_and_unsoeld(sh, oracle_mod):
         dens = (out[l * l : (l + 1) ** 2] ** 2).sum(dim=0)
         bound = 2 * np.sqrt((2 * l + 1) / (4 * np.pi)) * np.sqrt(2 * l + 1) * TOL64
         assert float((dens - (2 * l + 1) / (4 * np.pi)).abs().max()) <= bound, l
+
+
+# ----------------------------------------------------------------------------- point-range partition
+@pytest.mark.parametrize("n_total", [128**3, 128**3 - 5])
+def test_point_range_shards_are_bit_identical_to_the_single_call(sh, n_total):
+    """The multi-GPU scheme is a contiguous point-range partition with no collective: what rank r of 8
+    would compute on its shard must be bit-identical to the same points of the unsharded call.  AoS: each shard writes its
+    row slice of ONE buffer; SoA: per-shard [K][N_g] blocks.  n_total = 128^3 - 5 gives shards of 262,143 points (odd N_g:
+    the SoA planes lose 16-byte alignment and fall off the tensor-store path) next to even ones."""
+    import torch
+
+    from paper_2510_05282_b200 import inputs
+
+    pts = inputs.config3_full_grid()[:n_total]
+    x = torch.from_numpy(pts).cuda()
+    whole_aos = sh.sh_real(x, 9, layout="aos")
+    whole_soa = sh.sh_real(x, 9, layout="soa")
+    sharded_aos = torch.full_like(whole_aos, float("nan"))
+    sizes = set()
+    for rank in range(8):
+        lo, hi = inputs.shard_range(n_total, rank, 8)
+        sizes.add(hi - lo)
+        xs = x[lo:hi]   # a contiguous row range of the device array: no copy
+        sh.sh_real(xs, 9, out=sharded_aos[lo:hi], layout="aos")
+        block = sh.sh_real(xs, 9, layout="soa")
+        assert torch.equal(block, whole_soa[:, lo:hi]), rank
+    torch.cuda.synchronize()
+    assert torch.equal(sharded_aos, whole_aos)
+    assert (n_total % 8 == 0) or any(sz % 2 for sz in sizes)
 
 
 # ----------------------------------------------------------------------------- north_star's bandwidth target

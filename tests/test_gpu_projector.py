@@ -142,10 +142,10 @@ def test_aos_store_modes(sh, oracle_mod, proj_l):
                     assert np.abs(got - want).max() <= TOL * max(1.0, np.abs(tab).max()), (n, mis, mode, split)
 
 
-@pytest.mark.parametrize("form", [0, 1])
+@pytest.mark.parametrize("form", [1, 2])
 def test_project_polynomial_forms_value_by_value(sh, oracle_mod, form):
-    """sh_project has two polynomial forms (`project_form` knob): the factorized ones (0) and Horner in z^2 + the
-    (x + iy)^m recurrence (1).  One-hot weight vectors turn the projection into the per-point values (every other term
+    """sh_project has two polynomial forms (`project_form` knob): Horner in z^2 + the (x + iy)^m recurrence (1, the
+    default of this FP64-bound call) and the factorized forms of every other call (2).  One-hot weight vectors turn the projection into the per-point values (every other term
     of the sum is an exact 0), so each form is checked VALUE BY VALUE against the oracle at the fp64 tolerance: random
     directions, points within 1e-6 of the poles and the axes, the origin, points beyond the table."""
     rng = np.random.default_rng(17)
@@ -173,15 +173,16 @@ def test_project_polynomial_forms_value_by_value(sh, oracle_mod, form):
 
 
 @pytest.mark.parametrize("nvec", [1, 4])
-def test_project_fast_forms_full_grid(sh, oracle_mod, nvec):
-    """The Horner / recurrence forms on the bench's FP64-bound workload (128^3 grid, 100 columns) against the oracle's sum."""
+def test_project_factorized_forms_full_grid(sh, oracle_mod, nvec):
+    """The factorized forms (knob value 2; the default is Horner / recurrence) on the bench's FP64-bound workload (128^3 grid,
+    100 columns) against the oracle's sum."""
     from paper_2510_05282_b200 import inputs
 
     pts = inputs.config3_full_grid()
     proj_l, tab, dr = inputs.projector_channels(lmax=9, per_l=1, cutoff=6.0, dr=0.02)
     w = inputs.wave_weights(len(pts), nvec, seed=8, volume_element=(12.0 / 128) ** 3)
     coeff, abs_sum = oracle_mod.project(pts, proj_l, tab, dr, w)
-    sh.set_tuning("project_form", 1)
+    sh.set_tuning("project_form", 2)
     try:
         got = gpu_project(sh, pts, proj_l, tab, dr, w)
     finally:

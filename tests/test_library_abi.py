@@ -121,3 +121,38 @@ def test_generator_output_is_current():
     generate.self_check_recurrence()
     path = os.path.join(ROOT, "paper_2510_05282_b200", "csrc", "sh_generated.cuh")
     assert open(path).read() == generate.emit()
+
+
+def test_peaks_library_exports_its_entry_points():
+    """csrc/sh_peaks.cu -> libshb200_peaks.so: the ceilings microbenchmarks bench.py measures in the same run (no launch here)."""
+    from paper_2510_05282_b200 import build, peaks
+
+    build.build_peaks()
+    lib = peaks.load()
+    for name in ("shpeak_fill_flat", "shpeak_fill_bulk_tiles", "shpeak_fill_soa_planes", "shpeak_dfma"):
+        assert hasattr(lib, name), name
+    assert lib.shpeak_fill_flat(None, 64, None) == -1 and lib.shpeak_fill_bulk_tiles(None, 64, 16, None) == -1
+    assert lib.shpeak_fill_soa_planes(None, 64, 4, 32, 4, None) == -1 and lib.shpeak_dfma(None, 1, 1, None) == -1
+
+
+def test_host_call_validates_buffers_before_the_library_sees_them(lib):
+    """binding.host_call: a wrong dtype, a strided or too-small `out` must raise instead of letting sh_*_host write out of bounds."""
+    import torch
+
+    import paper_2510_05282_b200 as sh
+
+    pts = np.zeros((5, 3))
+    with pytest.raises(ValueError):
+        sh.host_call("real", pts, 3, out=np.empty((5, 16), dtype=np.float32))
+    with pytest.raises(ValueError):
+        sh.host_call("real", pts, 3, out=np.empty((5, 15)))
+    with pytest.raises(ValueError):
+        sh.host_call("real", pts, 3, out=np.empty((5, 32))[:, ::2])
+    with pytest.raises(ValueError):
+        sh.host_call("real", np.zeros((5, 2)), 3)
+    with pytest.raises(ValueError):
+        sh.host_call("real", torch.zeros((5, 3), dtype=torch.float32), 3)
+    with pytest.raises(ValueError):
+        sh.host_call("real", torch.zeros((5, 3), dtype=torch.float64), 3, out=torch.zeros((5, 16), dtype=torch.float64)[:, ::2])
+    with pytest.raises(ValueError):
+        sh.host_call("real_f32", torch.zeros((5, 3), dtype=torch.float32), 3, out=torch.zeros(5 * 16 - 1, dtype=torch.float32))
