@@ -476,11 +476,12 @@ def projector_cases(sh, dev, timed, timed_graph, want, ceil=None):
             if n < (1 << 18):
                 res[f"project nvec={nvec} {name}"].update({"ms": ms_py, "ms_in_cuda_graph": ms})
             else:
-                # the same call with the Horner / recurrence forms (SH_TUNE_PROJECT_FORM = 1): the factorized-vs-Horner
-                # question of the paper in the one place where arithmetic, not HBM, sets the time
-                sh.set_tuning("project_form", 1)
+                # the same call with the factorized root-pair forms of every other call (SH_TUNE_PROJECT_FORM = 2; the default
+                # of this one FP64-bound call is Horner in z^2 + the azimuthal recurrence): the factorized-vs-Horner question of
+                # the paper in the one place where arithmetic, not HBM, sets the time
+                sh.set_tuning("project_form", 2)
                 try:
-                    res[f"project nvec={nvec} {name}"]["ms_horner_recurrence_forms"] = timed(
+                    res[f"project nvec={nvec} {name}"]["ms_factorized_forms"] = timed(
                         lambda: sh.sh_project(x, proj_l, t, dr, w, coeff=coeff, workspace=ws), reps)
                 finally:
                     sh.set_tuning("project_form", 0)
