@@ -433,7 +433,7 @@ def projector_cases(sh, dev, timed, timed_graph, want, ceil=None):
         ("128^3 grid l9 x1 channel (100 cols)", inputs.config3_full_grid(), (9, 1, 6.0, 0.02), (12.0 / 128) ** 3),
     ]
     for name, pts, (lmax, per_l, cutoff, dr), dv in work:
-        if not any(want(f"{k} {name}") for k in ("projectors soa", "projectors aos", "project nvec=1", "project nvec=4")):
+        if not any(want(f"{k} {name}") for k in ("projectors soa", "projectors aos", "project nvec=1", "project nvec=4", "project nvec=8")):
             continue
         n = len(pts)
         proj_l, tab, dr = inputs.projector_channels(lmax=lmax, per_l=per_l, cutoff=cutoff, dr=dr)
@@ -454,7 +454,7 @@ def projector_cases(sh, dev, timed, timed_graph, want, ceil=None):
             if n < (1 << 18):
                 res[f"projectors {layout} {name}"]["ms_in_cuda_graph"] = timed_graph(lambda: sh.sh_projectors(x, proj_l, t, dr, out=out, layout=layout), 100)
             del out
-        for nvec in (1, 4):
+        for nvec in (1, 4, 8):
             if not want(f"project nvec={nvec} {name}"):
                 continue
             w = torch.from_numpy(inputs.wave_weights(n, nvec, seed=8, volume_element=dv)).to(dev)

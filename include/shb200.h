@@ -133,7 +133,8 @@ int sh_lmax_ext(void);
  *   w = psi dV; NOTHING per point is written.  The sum is taken in a fixed order (per-CTA partial sums in `workspace`,
  *   then one ordered pass), so results are reproducible run to run on one device; they differ from the sum in point
  *   order by rounding only (<= 1e-12 sum_i |w_i beta_i| is the tested bound).  `workspace` must hold at least
- *   sh_project_workspace_bytes(ncols, nvec) bytes, 8-byte aligned; its contents are scratch. */
+ *   sh_project_workspace_bytes(ncols, nvec) bytes, 8-byte aligned; its contents are scratch.  One pass over the points
+ *   serves up to 8 weight vectors and 104 columns (whole channels); more vectors or columns run as several passes. */
 enum { SH_MAX_PROJ = 32 };
 int sh_projector_count(int nproj, const int* proj_l);            /* ncols, or -1 if a proj_l is outside [0, 9] or nproj outside [0, 32] */
 int64_t sh_project_workspace_bytes(int ncols, int nvec);        /* -1 on bad arguments */

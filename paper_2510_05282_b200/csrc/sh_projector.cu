@@ -16,6 +16,9 @@ struct ProjPlan {
     double inv_dr;
     unsigned char first[shgen::LMAX_CAP + 2];   // channel slots of block l: [first[l], first[l+1])  (slots sorted by l)
     unsigned char chan[SH_MAX_PROJ];       // slot -> row of `radial`
+    unsigned char part_first[5];           // sh_project: slots of warp part p are part_slots[part_first[p] .. part_first[p+1])
+    unsigned char part_slots[SH_MAX_PROJ];
+    int row[SH_MAX_PROJ];                  // slot -> offset of its row in `radial` (chan * nr)
     unsigned short col[SH_MAX_PROJ];       // slot -> first column of the channel in this launch's output
 };
 
@@ -31,23 +34,16 @@ struct RadialPos {
         j = in ? (int)t : 0;
         u = in ? t - (double)j : 0.0;
     }
+    __device__ __forceinline__ double f_row(const double* __restrict__ tab) const {
+        const double a = __ldg(tab + j), b = __ldg(tab + j + 1);
+        return in ? fma(u, b - a, a) : 0.0;
+    }
     __device__ __forceinline__ double f(const double* __restrict__ radial, int nr, int channel) const {
         const double* tab = radial + (int64_t)channel * nr + j;
         const double a = __ldg(tab), b = __ldg(tab + 1);
         return in ? fma(u, b - a, a) : 0.0;
     }
 };
-
-// Radial values of EVERY channel slot at this lane's point, computed up front and parked in shared memory as
-// fs[slot*32 + lane] (times `scale`).  The table loads of different slots are independent, so their latencies overlap;
-// loaded one l-block at a time instead, a warp pays one dependent L2 round trip per channel (the staging tiles leave
-// little L1).  sh_project uses this; sh_proj_aos_kernel shares the slots among the warps of its tile the same way.
-__device__ __forceinline__ void stage_radial(const RadialPos& pos, const double* __restrict__ radial, const ProjPlan& plan, double* fs, int lane,
-                                             double scale) {
-    const int nslots = plan.first[shgen::LMAX_CAP + 1];
-#pragma unroll 4
-    for (int s = 0; s < nslots; ++s) fs[s * 32 + lane] = pos.f(radial, plan.nr, plan.chan[s]) * scale;
-}
 
 // the real harmonics of block l in ascending m (a3-a5), handed to the sink one block at a time
 // FAST: Horner-in-z^2 polar factors and the azimuthal recurrence instead of the factorized forms -- ~35 % fewer FP64
@@ -197,27 +193,25 @@ __global__ void __launch_bounds__(32 * SPLIT) sh_proj_aos_kernel(const double* _
     }
 }
 
-// sh_project: coeff[v][col] = sum_i w[v][i] beta_col(r_i).  Nothing per point is written, so the FP64 pipe is the bound.
-// One warp = one 32-point tile at a time, tiles dealt round-robin over all warps of a grid that fills the machine once;
-// the next tile's point and weights are loaded before the current tile is evaluated.  The l-blocks a lane produces are
-// staged, scaled by the radial values, in SEGMENTS of at most 32 columns (whole channels, packed in the order of
-// production; segment plan in ProjSegments) in the warp's shared-memory tile, TRANSPOSED: tile[column][point], pitch 34
-// doubles, so a lane's staging stores are conflict-free 8-byte stores (32 consecutive doubles per column) and, when a
-// segment is complete, lane c sums column c over the 32 points with 16-byte loads (rows 272 B apart: eight lanes per
-// 128-byte wavefront, conflict-free) and adds the result to the warp's running sums in shared memory.
-//   NV = 1: the weight is folded into the radial value (beta w is staged), the column sum is 32 additions;
-//   NV = 4: up to four weight vectors; the tile's weights sit in shared memory as [point][4] and are read as broadcasts.
-// Idle lanes of a ragged last tile evaluate the point (0, 0, 1) with weight 0, so every column sum runs over 32 rows.
-// Running sums are kept in the order of production ("slot order"); at the end a CTA adds its four warps in a fixed order
-// and writes one row of `partial` [cta][nvec][ncols]; sh_project_reduce_kernel adds the rows in a fixed order and
-// scatters to the caller's column order.
-constexpr int PROJ_CTAS_NV1 = 4, PROJ_CTAS_NV4 = 3;   // resident CTAs per SM (__launch_bounds__): register budget
-constexpr int PROJ_NV = 4;          // weight vectors contracted per launch
-constexpr int PROJ_MAX_COLS = 128;  // columns per launch (whole channels); wider channel lists run as several launches
+constexpr int PROJ_NV = 8;           // weight vectors contracted per launch
+constexpr int PROJ_MAX_COLS = 104;   // columns per launch (whole channels); wider channel lists run as several launches
+constexpr int PROJ_RING_MAX = 8;     // tile slots in flight (ring kernel)
+
+// ------------------------------------------------------------------------------------------------
+// sh_project with ONE weight vector: sh_project_seg_kernel.  One warp = one 32-point tile at a time, tiles dealt round-robin
+// over all warps of a grid that fills the machine once; the next tile's point and weight are loaded before the current tile is
+// evaluated.  The weight is folded into the radial values (w beta is what a lane produces), so the contraction is a plain column
+// sum: the l-blocks are staged in SEGMENTS of at most 32 columns (whole channels, packed in the order of production; plan in
+// ProjSegments) in the warp's shared-memory tile, TRANSPOSED: tile[column][point], pitch 34 doubles, so a lane's staging stores are
+// conflict-free 8-byte stores and, when a segment is complete, lane c sums column c over the 32 points with 16-byte loads (rows
+// 272 B apart: conflict-free) and adds the result to the warp's running sums in shared memory.  With one vector this beats the
+// ring kernel below (0.158 vs 0.175 ms on the 128^3 grid, 100 columns): there is no weight traffic to save, and sixteen warps each
+// own a whole tile.  Idle lanes of a ragged last tile evaluate the point (0, 0, 1) with weight 0.  Running sums are kept in the
+// order of production ("slot order"); at the end a CTA adds its four warps in a fixed order and writes one row of `partial`
+// [cta][ncols] in the caller's column order.
+constexpr int PROJ_SEG_CTAS = 4;    // resident CTAs per SM (__launch_bounds__): register budget
 constexpr int PROJ_SEG_PITCH = 34;  // doubles between consecutive columns of the transposed segment tile
-template <int NV> constexpr int project_smem_doubles_per_warp() {
-    return 32 * PROJ_SEG_PITCH + NV * PROJ_MAX_COLS + (NV > 1 ? 32 * PROJ_NV : 0);   // tile, running sums, weights
-}
+constexpr int project_seg_doubles_per_warp() { return 32 * PROJ_SEG_PITCH + PROJ_MAX_COLS; }   // tile, running sums
 
 struct ProjSegments {
     unsigned short scol[SH_MAX_PROJ];   // slot -> its first column in slot order
@@ -225,13 +219,19 @@ struct ProjSegments {
     unsigned char flush[SH_MAX_PROJ];   // slot -> 1 if the segment is complete after this slot
 };
 
-// column sums of a complete segment, added to the warp's running sums
-template <int NV>
-__device__ __forceinline__ void project_flush(double* tile, double* sums, const double* wt, int lane, int begin, int len) {
-    __syncwarp();
-    if (lane < len) {
-        const double2* t = reinterpret_cast<const double2*>(tile + lane * PROJ_SEG_PITCH);
-        if constexpr (NV == 1) {
+struct ProjectSegSink {
+    double* tile;        // the warp's [32][PROJ_SEG_PITCH] transposed segment tile
+    double* sums;        // the warp's running sums [PROJ_MAX_COLS]
+    const double* fs;    // this lane's radial values times its weight: fs[slot*32]
+    const ProjPlan& plan;
+    const ProjSegments& seg;
+    int lane;
+
+    // column sums of a complete segment, added to the warp's running sums
+    __device__ __forceinline__ void flush(int begin, int len) {
+        __syncwarp();
+        if (lane < len) {
+            const double2* t = reinterpret_cast<const double2*>(tile + lane * PROJ_SEG_PITCH);
             double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
 #pragma unroll
             for (int r = 0; r < 16; r += 2) {
@@ -239,46 +239,8 @@ __device__ __forceinline__ void project_flush(double* tile, double* sums, const 
                 s0 += a.x; s1 += a.y; s2 += b.x; s3 += b.y;
             }
             sums[begin + lane] += (s0 + s1) + (s2 + s3);
-        } else {
-            const double2* wv = reinterpret_cast<const double2*>(wt);   // row r: (w0, w1), (w2, w3)
-            double e[PROJ_NV], o[PROJ_NV];
-            static_for<0, PROJ_NV>([&](auto vc) { e[decltype(vc)::value] = 0.0; o[decltype(vc)::value] = 0.0; });
-#pragma unroll
-            for (int r = 0; r < 16; ++r) {
-                const double2 a = t[r];   // points 2r, 2r+1
-                const double2 w01 = wv[4 * r], w23 = wv[4 * r + 1], x01 = wv[4 * r + 2], x23 = wv[4 * r + 3];
-                e[0] = fma(a.x, w01.x, e[0]); e[1] = fma(a.x, w01.y, e[1]); e[2] = fma(a.x, w23.x, e[2]); e[3] = fma(a.x, w23.y, e[3]);
-                o[0] = fma(a.y, x01.x, o[0]); o[1] = fma(a.y, x01.y, o[1]); o[2] = fma(a.y, x23.x, o[2]); o[3] = fma(a.y, x23.y, o[3]);
-            }
-            static_for<0, PROJ_NV>([&](auto vc) {
-                constexpr int V = decltype(vc)::value;
-                sums[V * PROJ_MAX_COLS + begin + lane] += e[V] + o[V];
-            });
         }
-    }
-    __syncwarp();
-}
-
-__device__ __noinline__ void project_flush_call(double* tile, double* sums, const double* wt, int lane, int begin, int len) {
-    project_flush<PROJ_NV>(tile, sums, wt, lane, begin, len);
-}
-
-template <int NV>
-struct ProjectSink {
-    double* tile;        // the warp's [32][PROJ_SEG_PITCH] transposed segment tile
-    double* sums;        // the warp's running sums [NV][PROJ_MAX_COLS]
-    const double* wt;    // NV > 1: the tile's weights [32][PROJ_NV]
-    const double* fs;    // this lane's radial values fs[slot*32] (NV = 1: times the lane's weight)
-    const ProjPlan& plan;
-    const ProjSegments& seg;
-    int lane;
-
-    // NV = 4: out of line.  Inlined after every l-block its 210 instructions stand ten times in code that a warp runs through
-    // once per tile (4744 -> 2552 SASS instructions at lmax 9; 0.334 -> 0.327 ms on the 128^3 grid).  The 36 instructions of
-    // NV = 1 stay inline (the call costs more than the fetches: 0.189 -> 0.202 ms out of line).
-    __device__ __forceinline__ void flush(int begin, int len) {
-        if constexpr (NV == 1) project_flush<1>(tile, sums, wt, lane, begin, len);
-        else project_flush_call(tile, sums, wt, lane, begin, len);
+        __syncwarp();
     }
 
     template <int L> __device__ __forceinline__ void block(const double (&blk)[2 * L + 1]) {
@@ -293,34 +255,30 @@ struct ProjectSink {
     }
 };
 
-template <int LMAX, int NV, bool FAST>
-__global__ void __launch_bounds__(128, NV == 1 ? PROJ_CTAS_NV1 : PROJ_CTAS_NV4) sh_project_kernel(const double* __restrict__ xyz, int64_t n, const double* __restrict__ radial,
-                                                                          const __grid_constant__ ProjPlan plan, const __grid_constant__ ProjSegments seg,
-                                                                          const double* __restrict__ w, int nvec, double* __restrict__ partial) {
+template <int LMAX, bool FAST>
+__global__ void __launch_bounds__(128, PROJ_SEG_CTAS) sh_project_seg_kernel(const double* __restrict__ xyz, int64_t n, const double* __restrict__ radial,
+                                                                            const __grid_constant__ ProjPlan plan, const __grid_constant__ ProjSegments seg,
+                                                                            const double* __restrict__ w, double* __restrict__ partial) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nslots = plan.first[shgen::LMAX_CAP + 1];
-    double* s_tile = reinterpret_cast<double*>(smem_raw) + (size_t)warp * (project_smem_doubles_per_warp<NV>() + 32 * nslots);
+    const size_t wstride = project_seg_doubles_per_warp() + 32 * nslots;
+    double* s_tile = reinterpret_cast<double*>(smem_raw) + (size_t)warp * wstride;
     double* s_sums = s_tile + 32 * PROJ_SEG_PITCH;
-    double* s_wt = s_sums + NV * PROJ_MAX_COLS;
-    double* s_fs = s_tile + project_smem_doubles_per_warp<NV>();   // radial values [slot][lane]
+    double* s_fs = s_tile + project_seg_doubles_per_warp();   // radial values [slot][lane]
     const int ncols = plan.ncols;
-    for (int e = lane; e < NV * PROJ_MAX_COLS; e += 32) s_sums[e] = 0.0;
+    for (int e = lane; e < PROJ_MAX_COLS; e += 32) s_sums[e] = 0.0;
     const int64_t ntiles = (n + 31) >> 5;
     const int64_t gw = (int64_t)blockIdx.x * 4 + warp, nw = (int64_t)gridDim.x * 4;
-    struct Item { double x, y, z, w[NV]; };
+    struct Item { double x, y, z, w; };
     auto load = [&](int64_t t, Item& it) {
         const int64_t i = (t << 5) + lane;
         if (i < n) {
             const double* p = xyz + 3 * i;
             it.x = __ldg(p); it.y = __ldg(p + 1); it.z = __ldg(p + 2);
-            static_for<0, NV>([&](auto vc) {
-                constexpr int V = decltype(vc)::value;
-                it.w[V] = V < nvec ? __ldg(w + (int64_t)V * n + i) : 0.0;
-            });
+            it.w = __ldg(w + i);
         } else {   // idle lane of the ragged last tile: a harmless point with weight 0
-            it.x = 0.0; it.y = 0.0; it.z = 1.0;
-            static_for<0, NV>([&](auto vc) { it.w[decltype(vc)::value] = 0.0; });
+            it.x = 0.0; it.y = 0.0; it.z = 1.0; it.w = 0.0;
         }
     };
     Item cur, nxt;
@@ -328,35 +286,229 @@ __global__ void __launch_bounds__(128, NV == 1 ? PROJ_CTAS_NV1 : PROJ_CTAS_NV4) 
     if (t < ntiles) load(t, cur);
     for (; t < ntiles; t += nw) {
         if (t + nw < ntiles) load(t + nw, nxt);
-        if constexpr (NV > 1) {
-            // the previous tile's last column sum ended with __syncwarp: the weights may be overwritten
-            reinterpret_cast<double2*>(s_wt)[2 * lane] = make_double2(cur.w[0], cur.w[1]);
-            reinterpret_cast<double2*>(s_wt)[2 * lane + 1] = make_double2(cur.w[2], cur.w[3]);
-        }
         const RadialPos pos(cur.x, cur.y, cur.z, plan);
-        stage_radial(pos, radial, plan, s_fs, lane, NV == 1 ? cur.w[0] : 1.0);   // only this lane reads its column back
-        ProjectSink<NV> sink{s_tile, s_sums, s_wt, s_fs + lane, plan, seg, lane};
+        // radial values of EVERY channel slot, times the lane's weight, computed up front (independent table loads overlap; loaded one
+        // l-block at a time a warp pays one dependent L2 round trip per channel) and parked as fs[slot*32 + lane]
+#pragma unroll 4
+        for (int s = 0; s < nslots; ++s) s_fs[s * 32 + lane] = pos.f_row(radial + plan.row[s]) * cur.w;
+        ProjectSegSink sink{s_tile, s_sums, s_fs + lane, plan, seg, lane};
         eval_projector_blocks<LMAX, FAST>(normalize(cur.x, cur.y, cur.z), plan, sink);
         cur = nxt;
     }
-    // the CTA's four warps are added in a fixed order: one row of `partial` per CTA
+    // the CTA's four warps are added in a fixed order: one row of `partial` per CTA, in the caller's column order
     __syncthreads();
-    const size_t wstride = project_smem_doubles_per_warp<NV>() + 32 * nslots;
     const double* s0 = reinterpret_cast<const double*>(smem_raw) + 32 * PROJ_SEG_PITCH;
-    for (int e = threadIdx.x; e < nvec * ncols; e += 128) {
-        const int v = e / ncols, c = e - v * ncols;
-        const double* q = s0 + v * PROJ_MAX_COLS + c;
-        partial[(int64_t)blockIdx.x * nvec * ncols + e] = ((q[0] + q[wstride]) + q[2 * wstride]) + q[3 * wstride];
+    for (int c = threadIdx.x; c < ncols; c += 128) {
+        const double* q = s0 + c;
+        int slot = 0;
+        while (slot + 1 < nslots && seg.scol[slot + 1] <= c) ++slot;   // slot-order column -> the caller's column
+        partial[(int64_t)blockIdx.x * ncols + plan.col[slot] + (c - seg.scol[slot])] = ((q[0] + q[wstride]) + q[2 * wstride]) + q[3 * wstride];
     }
 }
 
-// coeff[v*coeff_stride + user column] = sum over CTAs of partial[cta][v][slot-order column], the rows added in a fixed
-// order (reproducible): 32 lanes = 32 consecutive (v, column) elements; the block's 32 warps each add every 32nd row of
-// `partial` (coalesced, four loads in flight), then the 32 sums are added in order.
-__global__ void __launch_bounds__(1024) sh_project_reduce_kernel(const double* __restrict__ partial, int nrows, int nvec, const __grid_constant__ ProjPlan plan,
-                                                                  const __grid_constant__ ProjSegments seg, double* __restrict__ coeff, int coeff_stride) {
+// sh_project with 2 to 8 weight vectors per launch: sh_project_kernel.  coeff[v][col] = sum_i w[v][i] beta_col(r_i).  Nothing per point is written, so the FP64 pipe is the bound --
+// provided the contraction does not spend the shared-memory bandwidth first (the previous design transposed every tile
+// through shared memory and re-read the tile's weights as broadcasts per 32-column segment: ~710 shared-memory wavefronts
+// per tile against 500 FP64-pipe cycles).  Here a lane IS a point on both sides of the hand-off, so nothing is transposed:
+//
+//   one persistent CTA per SM = NPW producer warps + NCW consumer warps around a ring of tile slots in shared memory
+//   (slot = vals[ncols][32] + wts[NV][32] doubles; mbarrier full/empty pair per slot).
+//   PRODUCERS: SPLIT warps share one 32-point tile (lane i = point i; warp `part` evaluates the l-blocks of block_part, a2/a3
+//     repeated) and stage beta_col = f_p(r) R_l^m at vals[col][lane] (conflict-free 8-byte stores); the tile's weights go to
+//     wts[v][lane].  The radial values of a warp's own channel slots are fetched up front (independent table loads overlap)
+//     and parked in the first column cell of each channel until the block is produced.
+//   CONSUMERS: every consumer warp visits every tile, but owns only some columns: a lane keeps acc[v][j] for its point
+//     position and its columns IN REGISTERS across all tiles of the CTA (acc += wts[v][lane] * vals[col][lane]: one 8-byte
+//     conflict-free load per NV FMAs, no broadcast, no transpose, every lane busy), and the cross-lane sum is taken once,
+//     at the end, by a butterfly.  The accumulators are what bounds the shape: NV x ncols x 32 lanes doubles per CTA
+//     (NV = 4, 104 columns: 26.6 K of the SM's 64 K registers), hence separate consumer warps that never evaluate a
+//     polynomial, and for NV = 8 lane GROUPS: G groups of 32/G lanes own different columns and take G points each per tile
+//     (group g reads the point quarters in the rotated order (k + g) % G, so the G groups hit different banks).
+//   The consumers' FMAs are independent and fill the FP64-pipe bubbles of the producers' dependent polynomial chains.
+// Tiles are dealt round-robin to the CTAs (static: the summation order is fixed, results are reproducible); idle lanes of a
+// ragged last tile stage the point (0, 0, 1) with weight 0.  One row of `partial` [cta][nvec][ncols] per CTA, then
+// sh_project_reduce_kernel adds the rows in a fixed order.
+
+template <int NV> struct ProjCfg;
+//                                   producer warps, warps per tile, consumer warps, lane groups per consumer warp
+// 20 warps = 640 threads leave 96 registers per thread: the producers' polynomial code needs them (at 80, with 16 + 8 warps, it spills
+// and a tile takes 7200 instead of 5700 cycles), and two consumer warps per scheduler get the issue share their FMAs need (with one,
+// the consumers, not the producers, set the time: 0.268 vs 0.247 ms for four vectors on the 128^3 grid).
+template <> struct ProjCfg<4> { static constexpr int NPW = 12, SPLIT = 2, NCW = 8, G = 2; };
+template <> struct ProjCfg<8> { static constexpr int NPW = 12, SPLIT = 2, NCW = 8, G = 4; };
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {   // release.cta
+    asm volatile("{\n.reg .b64 t;\nmbarrier.arrive.shared::cta.b64 t, [%0];\n}" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {   // acquire.cta
+    uint32_t done;
+    do {
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(done)
+                     : "r"(smem_u32(bar)), "r"(parity)
+                     : "memory");
+    } while (!done);
+}
+
+struct ProjectStage {
+    double* sv;   // the tile slot's vals + lane
+    const ProjPlan& plan;
+    template <int L> __device__ __forceinline__ void block(const double (&blk)[2 * L + 1]) {
+#pragma unroll 1   // code size is instruction-fetch traffic (see ProjRowSink)
+        for (int s = plan.first[L]; s < plan.first[L + 1]; ++s) {
+            double* q = sv + plan.col[s] * 32;
+            const double f = q[0];   // parked there by the radial pass
+            static_for<0, 2 * L + 1>([&](auto mc) { q[decltype(mc)::value * 32] = f * blk[decltype(mc)::value]; });
+        }
+    }
+};
+
+// The consumer side of sh_project_kernel for a warp whose lanes own R columns each (column owner + j * OWNERS, j < R).
+template <int NV, int G, int OWNERS, int R>
+__device__ __forceinline__ void project_consume(const double* ring, int slot_doubles, int nring, uint64_t* full, uint64_t* empty, int64_t my_tiles,
+                                                int ncols, int nvec, int cw, int lane, double* __restrict__ partial) {
+    constexpr int PTS = 32 / G;
+    const int g = lane / PTS, pl = lane % PTS;
+    const int owner = cw * G + g;
+    double acc[NV][R > 0 ? R : 1];
+    static_for<0, NV>([&](auto vc) { static_for<0, R>([&](auto jc) { acc[decltype(vc)::value][decltype(jc)::value] = 0.0; }); });
+    int slot = 0, use = 0;
+    for (int64_t seq = 0; seq < my_tiles; ++seq) {
+        mbar_wait(full + slot, use & 1);
+        if constexpr (R > 0) {
+            const double* sv = ring + (size_t)slot * slot_doubles;
+#pragma unroll
+            for (int k = 0; k < G; ++k) {
+                const int pt = pl + PTS * ((k + g) % G);   // rotated: the G groups read different banks
+                const double* wrow = sv + ncols * 32 + pt;
+                const double* col = sv + owner * 32 + pt;   // a lane whose owner has one column fewer reads a weights row in its last round: never written out
+                double wt[NV], val[R];
+                static_for<0, NV>([&](auto vc) { wt[decltype(vc)::value] = wrow[decltype(vc)::value * 32]; });
+                static_for<0, R>([&](auto jc) { val[decltype(jc)::value] = col[decltype(jc)::value * OWNERS * 32]; });
+                static_for<0, R>([&](auto jc) {
+                    static_for<0, NV>([&](auto vc) {
+                        acc[decltype(vc)::value][decltype(jc)::value] = fma(wt[decltype(vc)::value], val[decltype(jc)::value], acc[decltype(vc)::value][decltype(jc)::value]);
+                    });
+                });
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty + slot);
+        if (++slot == nring) { slot = 0; ++use; }
+    }
+    // sum over the group's lanes (butterfly: every lane ends with the same value), one row of `partial` per CTA
+    static_for<0, NV>([&](auto vc) {
+        constexpr int V = decltype(vc)::value;
+        static_for<0, R>([&](auto jc) {
+            constexpr int J = decltype(jc)::value;
+            double s = acc[V][J];
+#pragma unroll
+            for (int off = PTS / 2; off >= 1; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+            const int c = owner + J * OWNERS;
+            if (pl == 0 && c < ncols && V < nvec) partial[((int64_t)blockIdx.x * nvec + V) * ncols + c] = s;
+        });
+    });
+}
+
+template <int LMAX, int NV, bool FAST>
+__global__ void __launch_bounds__(32 * (ProjCfg<NV>::NPW + ProjCfg<NV>::NCW), 1)
+    sh_project_kernel(const double* __restrict__ xyz, int64_t n, const double* __restrict__ radial, const __grid_constant__ ProjPlan plan,
+                      const double* __restrict__ w, int nvec, double* __restrict__ partial, int nring) {
+    using Cfg = ProjCfg<NV>;
+    constexpr int NPW = Cfg::NPW, SPLIT = Cfg::SPLIT, NCW = Cfg::NCW, G = Cfg::G;
+    static_assert(NPW % SPLIT == 0 && 32 % G == 0 && NV >= G - 1, "shape");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int ncols = plan.ncols;
+    const int slot_doubles = (ncols + NV) * 32;
+    double* ring = reinterpret_cast<double*>(smem_raw);
+    uint64_t* full = reinterpret_cast<uint64_t*>(ring + (size_t)nring * slot_doubles);
+    uint64_t* empty = full + PROJ_RING_MAX;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < nring; ++s) {
+            mbar_init(full + s, SPLIT);   // one arrival per producer warp of the tile
+            mbar_init(empty + s, NCW);    // one per consumer warp
+        }
+    }
+    __syncthreads();
+    const int64_t ntiles = (n + 31) >> 5;
+    const int64_t my_tiles = (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x;   // tiles blockIdx.x + seq * gridDim.x
+
+    if (warp < NPW) {
+        // ---------------- producer ----------------
+        constexpr int STREAMS = NPW / SPLIT;
+        const int stream = warp / SPLIT, part = warp % SPLIT;
+        const int ps0 = plan.part_first[part], ps1 = plan.part_first[part + 1];   // this warp's channel slots
+        // point index of this lane in the stream's current tile; the stream advances by STREAMS * gridDim.x tiles
+        int64_t i = (((int64_t)blockIdx.x + (int64_t)stream * gridDim.x) << 5) + lane;
+        const int64_t istep = ((int64_t)STREAMS * gridDim.x) << 5;
+        auto load_point = [&](int64_t ip, double& x, double& y, double& z) {
+            const bool ok = ip < n;   // idle lane of the ragged last tile: a harmless point (its weights are 0)
+            const double* p = xyz + 3 * (ok ? ip : 0);
+            const double a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
+            x = ok ? a : 0.0; y = ok ? b : 0.0; z = ok ? c : 1.0;
+        };
+        double x = 0.0, y = 0.0, z = 1.0, nx = 0.0, ny = 0.0, nz = 1.0;
+        int64_t seq = stream;
+        if (seq < my_tiles) load_point(i, x, y, z);
+        int slot = stream % nring, use = stream / nring;
+        for (; seq < my_tiles; seq += STREAMS, i += istep) {
+            if (seq + STREAMS < my_tiles) load_point(i + istep, nx, ny, nz);
+            // the tile's weights: vector v is fetched by warp part v % SPLIT
+            constexpr int WPP = (NV + SPLIT - 1) / SPLIT;
+            double wv[WPP];
+            static_for<0, WPP>([&](auto kc) {
+                const int v = part + decltype(kc)::value * SPLIT;
+                wv[decltype(kc)::value] = (v < nvec && i < n) ? __ldg(w + (int64_t)v * n + i) : 0.0;
+            });
+            if (use > 0) mbar_wait(empty + slot, (use - 1) & 1);   // the consumers have released the slot's previous tile
+            double* sv = ring + (size_t)slot * slot_doubles + lane;
+            const RadialPos pos(x, y, z, plan);
+#pragma unroll 4
+            for (int k = ps0; k < ps1; ++k) {
+                const int s = plan.part_slots[k];
+                sv[plan.col[s] * 32] = pos.f_row(radial + plan.row[s]);
+            }
+            const UnitVec u = normalize(x, y, z);
+            ProjectStage sink{sv, plan};
+            static_for<0, SPLIT>([&](auto pc) {
+                constexpr int PART = decltype(pc)::value;
+                if (part == PART) eval_projector_blocks<LMAX, FAST, SPLIT, PART>(u, plan, sink);
+            });
+            static_for<0, WPP>([&](auto kc) {
+                const int v = part + decltype(kc)::value * SPLIT;
+                if (v < NV) sv[(ncols + v) * 32] = wv[decltype(kc)::value];
+            });
+            __syncwarp();
+            if (lane == 0) mbar_arrive(full + slot);
+            x = nx; y = ny; z = nz;
+            slot += STREAMS;
+            while (slot >= nring) { slot -= nring; ++use; }
+        }
+    } else {
+        // ---------------- consumer ----------------
+        constexpr int OWNERS = NCW * G, CPW = (PROJ_MAX_COLS + OWNERS - 1) / OWNERS;
+        const int cw = warp - NPW;
+        // column rounds of the warp's first owner (warp-uniform): the tile loop is compiled once per count, branch-free inside
+        const int rounds = (ncols - cw * G + OWNERS - 1) / OWNERS;
+        static_for<0, CPW + 1>([&](auto rc) {
+            constexpr int R = decltype(rc)::value;
+            if ((rounds < 0 ? 0 : rounds) == R)
+                project_consume<NV, G, OWNERS, R>(ring, slot_doubles, nring, full, empty, my_tiles, ncols, nvec, cw, lane, partial);
+        });
+    }
+}
+
+// coeff[v*coeff_stride + col] = sum over CTAs of partial[cta][v][col], the rows added in a fixed order (reproducible):
+// 32 lanes = 32 consecutive (v, column) elements; the block's 32 warps each add every 32nd row of `partial` (coalesced, four
+// loads in flight), then the 32 sums are added in order.
+__global__ void __launch_bounds__(1024) sh_project_reduce_kernel(const double* __restrict__ partial, int nrows, int nvec, int ncols,
+                                                                  double* __restrict__ coeff, int coeff_stride) {
     __shared__ double s[32][33];
-    const int ncols = plan.ncols, ne = nvec * ncols;
+    const int ne = nvec * ncols;
     const int y = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int e = blockIdx.x * 32 + lane;
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
@@ -375,12 +527,8 @@ __global__ void __launch_bounds__(1024) sh_project_reduce_kernel(const double* _
     if (y == 0 && e < ne) {
         double t = 0.0;
         for (int k = 0; k < 32; ++k) t += s[k][lane];
-        // slot-order column -> the caller's column
         const int v = e / ncols, c = e - v * ncols;
-        int slot = 0;
-        const int nslots = plan.first[shgen::LMAX_CAP + 1];
-        while (slot + 1 < nslots && seg.scol[slot + 1] <= c) ++slot;
-        coeff[v * coeff_stride + plan.col[slot] + (c - seg.scol[slot])] = t;
+        coeff[v * coeff_stride + c] = t;
     }
 }
 
@@ -415,6 +563,7 @@ int make_plan(const int* proj_l, int p0, int p1, int nr, double dr, ProjPlan& pl
         for (int p = p0; p < p1; ++p)
             if (proj_l[p] == l) {
                 plan.chan[slot] = (unsigned char)p;
+                plan.row[slot] = p * nr;
                 plan.col[slot] = (unsigned short)col0[p];
                 ++slot;
             }
@@ -431,7 +580,6 @@ int check_projector_args(const double* xyz, int64_t n, int nproj, const int* pro
     return SH_OK;
 }
 
-constexpr int PROJ_CTAS_PER_SM = PROJ_CTAS_NV1 > PROJ_CTAS_NV4 ? PROJ_CTAS_NV1 : PROJ_CTAS_NV4;   // grid cap of sh_project_kernel: the machine filled once (what the workspace is sized for)
 
 // warps per tile (block_part): the default comes from the 128^3-grid measurements in DESIGN.md section 6
 constexpr int PROJ_AOS_SPLIT = 2;
@@ -523,46 +671,91 @@ void make_segments(const int* proj_l, const ProjPlan& plan, ProjSegments& seg) {
     if (nslots > 0) seg.flush[nslots - 1] = 1;
 }
 
+// channel slots of each warp part of sh_project_kernel's producers (block_part<SPLIT>)
+template <int SPLIT>
+void fill_parts(const int* proj_l, ProjPlan& plan) {
+    const int nslots = plan.first[shgen::LMAX_CAP + 1];
+    int k = 0;
+    for (int part = 0; part < SPLIT; ++part) {
+        plan.part_first[part] = (unsigned char)k;
+        for (int s = 0; s < nslots; ++s)
+            if (block_part<SPLIT>(proj_l[plan.chan[s]]) == part) plan.part_slots[k++] = (unsigned char)s;
+    }
+    for (int part = SPLIT; part < 5; ++part) plan.part_first[part] = (unsigned char)k;
+}
+
 int64_t project_workspace_bytes(int ncols, int nvec) {
     if (ncols < 0 || nvec < 0) return -1;
     const int64_t cols = ncols < PROJ_MAX_COLS ? ncols : PROJ_MAX_COLS, vecs = nvec < PROJ_NV ? nvec : PROJ_NV;
-    return (int64_t)sm_count() * PROJ_CTAS_PER_SM * vecs * cols * (int64_t)sizeof(double);   // one row per CTA of the largest grid
+    return (int64_t)sm_count() * PROJ_SEG_CTAS * vecs * cols * (int64_t)sizeof(double);   // one row per CTA of the largest grid
+}
+
+// one weight vector: the transposed-segment kernel; rows of `partial` = its CTAs
+template <int LMAX>
+int launch_project_seg(const double* xyz, int64_t n, const double* radial, const int* proj_l, const ProjPlan& plan, const double* w, double* partial,
+                       int64_t* rows, cudaStream_t st) {
+    ProjSegments seg;
+    make_segments(proj_l, plan, seg);
+    const bool fast = tuned(SH_TUNE_PROJECT_FORM, 1) != 2;   // Horner / recurrence forms (default) or the factorized ones (knob value 2)
+    const int nslots = plan.first[shgen::LMAX_CAP + 1];
+    const size_t smem = (size_t)4 * (project_seg_doubles_per_warp() + 32 * nslots) * sizeof(double);   // 38 KB + 1 KB per slot
+    constexpr size_t smem_max = (size_t)4 * (project_seg_doubles_per_warp() + 32 * SH_MAX_PROJ) * sizeof(double);
+    auto launch = [&](auto kern, SmemOptIn& opted_in) -> int {
+        if (const int rc = ensure_dynamic_smem(kern, smem_max, opted_in); rc != SH_OK) return rc;
+        // the grid fills the machine once: resident CTAs per SM for THIS shared-memory size (228 KB per SM, 1 KB reserved per CTA;
+        // registers allow PROJ_SEG_CTAS): many channel slots leave fewer, and tiles are dealt statically, so a CTA that is not
+        // resident from the start would run as a second wave
+        int occ = (int)((size_t)228 * 1024 / (smem + 1024));
+        if (occ < 1) occ = 1;
+        if (occ > PROJ_SEG_CTAS) occ = PROJ_SEG_CTAS;
+        const int64_t ntiles = (n + 31) / 32, cap = (int64_t)sm_count() * occ;
+        int64_t blocks = (ntiles + 3) / 4;
+        if (blocks > cap) blocks = cap;
+        *rows = blocks;
+        kern<<<(unsigned)blocks, 128, smem, st>>>(xyz, n, radial, plan, seg, w, partial);
+        return launch_status();
+    };
+    static SmemOptIn opted_in[2];
+    return fast ? launch(sh_project_seg_kernel<LMAX, true>, opted_in[1]) : launch(sh_project_seg_kernel<LMAX, false>, opted_in[0]);
+}
+
+// 2 to 8 weight vectors: the ring kernel, one persistent CTA per SM; rows of `partial` = its CTAs
+template <int LMAX, int NV>
+int launch_project_ring(const double* xyz, int64_t n, const double* radial, const ProjPlan& plan, const double* w, int nvec, double* partial,
+                        int64_t* rows, cudaStream_t st) {
+    using Cfg = ProjCfg<NV>;
+    static_assert(Cfg::SPLIT == 2, "fill_parts<2> in run_project");
+    // ring of tile slots: as many as fit (at most PROJ_RING_MAX), then the 2 x PROJ_RING_MAX mbarriers
+    const size_t slot_bytes = (size_t)(plan.ncols + NV) * 32 * sizeof(double);
+    int nring = (int)(((size_t)227 * 1024 - 2 * PROJ_RING_MAX * sizeof(uint64_t)) / slot_bytes);
+    if (nring > PROJ_RING_MAX) nring = PROJ_RING_MAX;
+    if (nring < 1) return SH_ERR_PROJECTOR;
+    const size_t smem = (size_t)nring * slot_bytes + 2 * PROJ_RING_MAX * sizeof(uint64_t);
+    const bool fast = tuned(SH_TUNE_PROJECT_FORM, 1) != 2;
+    const int64_t ntiles = (n + 31) / 32;
+    const int64_t blocks = ntiles < sm_count() ? ntiles : sm_count();
+    *rows = blocks;
+    auto launch = [&](auto kern, SmemOptIn& opted_in) -> int {
+        if (const int rc = ensure_dynamic_smem(kern, (size_t)227 * 1024, opted_in); rc != SH_OK) return rc;
+        kern<<<(unsigned)blocks, 32 * (Cfg::NPW + Cfg::NCW), smem, st>>>(xyz, n, radial, plan, w, nvec, partial, nring);
+        return launch_status();
+    };
+    static SmemOptIn opted_in[2];
+    return fast ? launch(sh_project_kernel<LMAX, NV, true>, opted_in[1]) : launch(sh_project_kernel<LMAX, NV, false>, opted_in[0]);
 }
 
 template <int LMAX>
-int launch_project(const double* xyz, int64_t n, const double* radial, const ProjPlan& plan, const ProjSegments& seg, const double* w, int nvec,
+int launch_project(const double* xyz, int64_t n, const double* radial, const int* proj_l, const ProjPlan& plan, const double* w, int nvec,
                    double* partial, double* coeff, int coeff_stride, cudaStream_t st) {
-    const int64_t ntiles = (n + 31) / 32;
-    int64_t blocks = (ntiles + 3) / 4;
-    const int64_t cap = (int64_t)sm_count() * (nvec == 1 ? PROJ_CTAS_NV1 : PROJ_CTAS_NV4);   // resident CTAs per SM (__launch_bounds__)
-    if (blocks > cap) blocks = cap;
-    // per warp: segment tile, running sums, (weights,) and the radial values of every slot: 38 / 54 KB + 1 KB per slot per CTA
-    const size_t slots_bytes = (size_t)4 * 32 * plan.first[shgen::LMAX_CAP + 1] * sizeof(double);
-    constexpr size_t smem_max = (size_t)4 * (project_smem_doubles_per_warp<PROJ_NV>() + 32 * SH_MAX_PROJ) * sizeof(double);   // 86 KB
-    const bool fast = tuned(SH_TUNE_PROJECT_FORM, 1) != 2;   // Horner / recurrence forms (default) or the factorized ones (knob value 2)
-    auto launch = [&](auto kern, size_t warp_doubles, SmemOptIn& opted_in) -> int {
-        if (const int rc = ensure_dynamic_smem(kern, smem_max, opted_in); rc != SH_OK) return rc;
-        kern<<<(unsigned)blocks, 128, (size_t)4 * warp_doubles * sizeof(double) + slots_bytes, st>>>(xyz, n, radial, plan, seg, w, nvec, partial);
-        return SH_OK;
-    };
-    static SmemOptIn opted_in[4];
+    int64_t rows = 0;
     int rc;
-    if (nvec == 1) {
-        rc = fast ? launch(sh_project_kernel<LMAX, 1, true>, project_smem_doubles_per_warp<1>(), opted_in[1])
-                  : launch(sh_project_kernel<LMAX, 1, false>, project_smem_doubles_per_warp<1>(), opted_in[0]);
-    } else {
-        rc = fast ? launch(sh_project_kernel<LMAX, PROJ_NV, true>, project_smem_doubles_per_warp<PROJ_NV>(), opted_in[3])
-                  : launch(sh_project_kernel<LMAX, PROJ_NV, false>, project_smem_doubles_per_warp<PROJ_NV>(), opted_in[2]);
-    }
+    if (nvec == 1) rc = launch_project_seg<LMAX>(xyz, n, radial, proj_l, plan, w, partial, &rows, st);
+    else if (nvec <= 4) rc = launch_project_ring<LMAX, 4>(xyz, n, radial, plan, w, nvec, partial, &rows, st);
+    else rc = launch_project_ring<LMAX, 8>(xyz, n, radial, plan, w, nvec, partial, &rows, st);
     if (rc != SH_OK) return rc;
-    g_launches.fetch_add(1, std::memory_order_relaxed);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e);
     const int elems = nvec * plan.ncols;
-    sh_project_reduce_kernel<<<(elems + 31) / 32, 1024, 0, st>>>(partial, (int)blocks, nvec, plan, seg, coeff, coeff_stride);
-    g_launches.fetch_add(1, std::memory_order_relaxed);
-    e = cudaGetLastError();
-    return e == cudaSuccess ? SH_OK : cuda_fail(e);
+    sh_project_reduce_kernel<<<(elems + 31) / 32, 1024, 0, st>>>(partial, (int)rows, nvec, plan.ncols, coeff, coeff_stride);
+    return launch_status();
 }
 
 int run_project(const double* xyz, int64_t n, int nproj, const int* proj_l, const double* radial, int nr, double dr, const double* w,
@@ -586,13 +779,12 @@ int run_project(const double* xyz, int64_t n, int nproj, const int* proj_l, cons
         int p1 = p0, cols = 0;
         while (p1 < nproj && cols + 2 * proj_l[p1] + 1 <= PROJ_MAX_COLS) cols += 2 * proj_l[p1++] + 1;
         ProjPlan plan;
-        ProjSegments seg;
         const int lmax = make_plan(proj_l, p0, p1, nr, dr, plan);
-        make_segments(proj_l, plan, seg);
+        fill_parts<2>(proj_l, plan);   // every ProjCfg uses two warps per tile
         for (int v0 = 0; v0 < nvec; v0 += PROJ_NV) {
             const int nv = nvec - v0 < PROJ_NV ? nvec - v0 : PROJ_NV;
             switch (lmax) {
-#define SH_CASE(L) case L: rc = launch_project<L>(xyz, n, radial, plan, seg, w + (int64_t)v0 * n, nv, partial, coeff + (int64_t)v0 * ncols + c0, ncols, st); break;
+#define SH_CASE(L) case L: rc = launch_project<L>(xyz, n, radial, proj_l, plan, w + (int64_t)v0 * n, nv, partial, coeff + (int64_t)v0 * ncols + c0, ncols, st); break;
                 SH_CASE(0) SH_CASE(1) SH_CASE(2) SH_CASE(3) SH_CASE(4) SH_CASE(5) SH_CASE(6) SH_CASE(7) SH_CASE(8) SH_CASE(9)
 #undef SH_CASE
             }

@@ -81,7 +81,7 @@ def test_projector_grid_values(sh, oracle_mod, grid2, layout):
     assert np.abs(got - want).max() <= TOL * max(1.0, np.abs(tab).max())
 
 
-@pytest.mark.parametrize("nvec", [1, 3, 4, 6])
+@pytest.mark.parametrize("nvec", [1, 2, 3, 4, 6, 8, 11])   # one vector: segment kernel; 2-4 and 5-8: ring kernel; 11 = 8 + 3 in two passes
 def test_projector_grid_projection(sh, oracle_mod, grid2, nvec):
     from paper_2510_05282_b200 import inputs
 
