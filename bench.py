@@ -366,6 +366,22 @@ def extra_configs(sh, dev, only=None, ceil=None):
             "roofline": hbm_roofline(f"sh_real lmax=9 SoA, {coords} input", len(grid) * (arr.shape[1] * 8 + 8 * K), len(grid) * 8 * K, ms, peak, peak_src, ceil, "soa_planes")}
         del x
     del out
+    # the paper's own protocol (Table I: every harmonic evaluated, "accumulated and never stored"): bound by the FP64 pipe
+    fp64_peak = ceil["fp64_lane_ginstr_s"] if ceil else N_SMS * FP64_LANES_PER_SM * SM_MAX_GHZ
+    for coords, arr in (("cartesian", grid), ("normalized", unit), ("angular", ang)):
+        name = f"config3 real l9 compute-only sum (Table I protocol) {coords}"
+        if not want(name):
+            continue
+        x = torch.from_numpy(arr).to(dev)
+        o = torch.empty(len(grid), dtype=torch.float64, device=dev)
+        ms = timed(lambda: sh.sh_real_sum(x, LMAX, out=o, coords=coords), 20)
+        per_point = REAL_L9_FP64_PER_POINT + K if coords == "cartesian" else None   # a2-a5 + the K additions of the sum
+        res[name] = {"ms": ms, "G_values_per_s": len(grid) * K / ms / 1e6, "G_points_per_s": len(grid) / ms / 1e6}
+        if per_point:
+            res[name]["roofline"] = {"bound": "alu", "unit": "G FP64 lane-instr/s", "achieved": len(grid) * per_point / ms / 1e6, "peak": fp64_peak,
+                                     "frac": len(grid) * per_point / ms / 1e6 / fp64_peak, "fp64_instr_per_point": per_point,
+                                     "peak_source": "measured in this run (DFMA chains, csrc/sh_peaks.cu)" if ceil else "nominal 148 SMs x 64 lanes x 1.965 GHz"}
+        del x, o
     cases = [
         ("config1 real l4 SoA N=10008", "real", inputs.config1_cube(), 4, ["soa"], 50),
         ("config2 real l3 SoA N=113102", "real", inputs.config2_projector_grid(), 3, ["soa"], 50),
@@ -495,6 +511,7 @@ def projector_cases(sh, dev, timed, timed_graph, want, ceil=None):
 # compiled for the store kernels (cuobjdump: 94 at lmax = 3, 566 at lmax = 9), plus the radial position (sqrt, ~12) and the
 # table interpolation (3 per channel: 8 / 10 channels); DESIGN.md section 6.  Keys = lmax.
 PROJECT_FP64_PER_POINT = {3: 94 + 12 + 24, 9: 566 + 12 + 30}
+REAL_L9_FP64_PER_POINT = 566   # a2-a5 at lmax = 9 in the factorized forms (the store kernels' SASS count)
 
 
 def run_ours(args):

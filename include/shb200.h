@@ -59,8 +59,9 @@ enum {
  * alignment allows.  A request the alignment does not allow returns SH_ERR_ALIGNMENT.  Results are identical
  * on every path (same arithmetic, different store mechanism). */
 enum {
-    SH_STORE_AUTO   = 0 << 8, /* sh_real SoA with even n >= 128 and a 16-byte aligned out: tiles of 128 points staged in shared memory and
-                                 written by one TMA tensor store each (cp.async.bulk.tensor.2d through a tensor map of out as [K][n]);
+    SH_STORE_AUTO   = 0 << 8, /* SoA with a 16-byte aligned out: sh_real (even n >= 128), sh_real_f32 (n a multiple of 4, >= 256) and sh_complex
+                                 (n >= 64) stage tiles of 128 / 256 / 64 points in shared memory and write each with one TMA tensor store
+                                 (cp.async.bulk.tensor.2d through a tensor map of out as [K][n]: rows of 1 KB);
                                  AoS with a 16-byte aligned out: SH_STORE_BULK; everything else: SH_STORE_DIRECT */
     SH_STORE_DIRECT = 1 << 8, /* per-thread st.global.cs; SoA: coalesced planes; AoS: smem transpose + coalesced stores */
     SH_STORE_BULK   = 2 << 8  /* AoS only, needs a 16-byte aligned out: rows staged in shared memory, written by TMA bulk copies
@@ -99,6 +100,13 @@ int sh_complex(const double* xyz, int64_t n, int lmax, double* out, int layout, 
 int sh_spinor(const double* xyz, int64_t n, int lmax, double* out, int layout, void* stream);
 /* fp32 variant of sh_real: fp32 in, fp32 out; the normalization runs in fp64, the polynomials in fp32. */
 int sh_real_f32(const float* xyz, int64_t n, int lmax, float* out, int layout, void* stream);
+
+/* The paper's own measurement protocol (Table I: "the results are accumulated and never stored"):
+ * out[i] = sum over all l <= lmax, m of R_l^m(xyz_i), one double per point, every harmonic evaluated exactly as in sh_real.
+ * With 32 bytes of traffic per point instead of 824 this call is bound by the FP64 pipe: it measures the arithmetic side of
+ * the roofline of the factorized formulas, and its rate is the one comparable with the paper's CPU / V100 figures.
+ * `coords` is one of SH_COORDS_* (no layout bits: there is one value per point); DEVICE pointers; asynchronous on `stream`. */
+int sh_real_sum(const double* xyz, int64_t n, int lmax, double* out, int coords, void* stream);
 
 /* Extension beyond the paper's explicit range (its conclusion: "could be easily extended using recurrence
  * relationships for higher values of l"): real / complex harmonics for all l <= lmax <= 32 (sh_lmax_ext()).
@@ -173,7 +181,7 @@ int sh_index_spinor(int l, int twoj, int twomj);
 enum {
     SH_TUNE_PREFETCH_WINDOW_POINTS = 0, /* points per burst of the L2 input prefetch (default 262144); 1 = prefetch off */
     SH_TUNE_PROJ_AOS_MODE = 1,      /* sh_projectors AoS copy-out: 1 = warp copy, 2 = one bulk copy per row, 3 = one per tile (when possible) */
-    SH_TUNE_SOA_TMA = 2,            /* SoA through TMA tensor stores (tiles staged in shared memory): 0 = when possible (default), 1 = never (per-thread streaming stores) */
+    SH_TUNE_SOA_TMA = 2,            /* SoA through TMA tensor stores (sh_real, sh_real_f32, sh_complex; tiles staged in shared memory): 0 = when possible (default), 1 = never (per-thread streaming stores) */
     SH_TUNE_PROJECT_FORM = 3,       /* sh_project polynomials: 0 = default; 1 = Horner in z^2 for the polar factors and (x + iy)^m by
                                        recurrence; 2 = the factorized root-pair forms of every other call */
     SH_TUNE_PROJ_AOS_SPLIT = 4,     /* sh_projectors AoS, lmax >= 4: warps that share one 32-point tile, each evaluating part of the l-blocks: 1, 2 (default) or 4 */

@@ -25,5 +25,6 @@ from .binding import (  # noqa: F401
     sh_real,
     sh_real_ext,
     sh_real_f32,
+    sh_real_sum,
     sh_spinor,
 )

@@ -54,6 +54,8 @@ def load() -> ctypes.CDLL:
             f.argtypes = [vp, i64, ci, vp, ci, vp]
             f.restype = ci
         lib.sh_lmax_ext.restype = ci
+        lib.sh_real_sum.argtypes = [vp, i64, ci, vp, ci, vp]
+        lib.sh_real_sum.restype = ci
         for name in ("sh_real", "sh_complex", "sh_spinor", "sh_real_f32"):
             f = getattr(lib, name)
             f.argtypes = [vp, i64, ci, vp, ci, vp]
@@ -183,6 +185,26 @@ def sh_spinor(xyz, lmax, out=None, layout="soa", store="auto", stream=None, coor
 def sh_real_f32(xyz, lmax, out=None, layout="soa", store="auto", stream=None, coords="cartesian"):
     """fp32 variant of sh_real (float32 in, float32 out)."""
     return _device_call("real_f32", xyz, lmax, out, layout, store, stream, coords)
+
+
+def sh_real_sum(xyz, lmax, out=None, stream=None, coords="cartesian"):
+    """out[i] = sum over l <= lmax, m of R_l^m(xyz_i): the accumulate-and-never-store protocol of the paper's Table I."""
+    import torch
+
+    width = 2 if coords == "angular" else 3
+    if not (xyz.is_cuda and xyz.dtype == torch.float64 and xyz.is_contiguous() and xyz.dim() == 2 and xyz.shape[1] == width):
+        raise ValueError(f"xyz must be a contiguous CUDA tensor [n][{width}] of float64")
+    n = xyz.shape[0]
+    if out is None:
+        out = torch.empty(n, dtype=torch.float64, device=xyz.device)
+    elif not (out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == n):
+        raise ValueError(f"out must be a contiguous CUDA float64 tensor with {n} elements")
+    s = torch.cuda.current_stream(xyz.device).cuda_stream if stream is None else int(stream)
+    with torch.cuda.device(xyz.device):
+        rc = load().sh_real_sum(xyz.data_ptr(), n, int(lmax), out.data_ptr(), _COORDS[coords], s)
+    if rc != 0:
+        raise ShError(rc, "sh_real_sum")
+    return out
 
 
 def sh_real_ext(xyz, lmax, out=None, layout="soa", store="auto", stream=None, coords="cartesian"):

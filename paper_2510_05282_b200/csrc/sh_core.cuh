@@ -284,23 +284,37 @@ __device__ __forceinline__ void complex_block(const Azim<LMAX, T>& az, T z, bool
     });
 }
 
+// block l of the complex harmonics, m = -l..l, from the azimuthal factors (MAZ >= L of them)
+template <int L, int MAZ, typename T, class Sink>
+__device__ __forceinline__ void complex_emit_block(const Azim<MAZ, T>& az, T z, bool origin, Sink& sink) {
+    static_assert(MAZ >= L, "azimuthal factors up to m = l");
+    T a[L + 1], b[L + 1];
+    complex_block<L>(az, z, origin, a, b, sink);
+    static_for<0, L>([&](auto jc) {
+        constexpr int M = L - decltype(jc)::value;
+        sink.template put2<L * (L + 1) - M>(a[M], -b[M]);
+    });
+    sink.template put2<L * (L + 1)>(a[0], T(0));
+    static_for<1, L + 1>([&](auto mc) {
+        constexpr int M = decltype(mc)::value;
+        if constexpr (M % 2) sink.template put2<L * (L + 1) + M>(-a[M], -b[M]);
+        else sink.template put2<L * (L + 1) + M>(a[M], b[M]);
+    });
+    sink.template end_l<L>();
+}
+
 template <int LMAX, typename T, class Sink>
 __device__ __forceinline__ void eval_complex(const Azim<LMAX, T>& az, T z, bool origin, Sink& sink) {
+    static_for<0, LMAX + 1>([&](auto lc) { complex_emit_block<decltype(lc)::value>(az, z, origin, sink); });
+}
+
+// warp part PART of SPLIT (block_part, as eval_real_part)
+template <int LMAX, int SPLIT, int PART, typename T, class Sink>
+__device__ __forceinline__ void eval_complex_part(T x, T y, T z, bool origin, Sink& sink) {
+    const Azim<part_mmax<SPLIT, PART, LMAX>(), T> az(x, y);
     static_for<0, LMAX + 1>([&](auto lc) {
         constexpr int L = decltype(lc)::value;
-        T a[L + 1], b[L + 1];
-        complex_block<L>(az, z, origin, a, b, sink);
-        static_for<0, L>([&](auto jc) {
-            constexpr int M = L - decltype(jc)::value;
-            sink.template put2<L * (L + 1) - M>(a[M], -b[M]);
-        });
-        sink.template put2<L * (L + 1)>(a[0], T(0));
-        static_for<1, L + 1>([&](auto mc) {
-            constexpr int M = decltype(mc)::value;
-            if constexpr (M % 2) sink.template put2<L * (L + 1) + M>(-a[M], -b[M]);
-            else sink.template put2<L * (L + 1) + M>(a[M], b[M]);
-        });
-        sink.template end_l<L>();
+        if constexpr (block_part<SPLIT>(L) == PART) complex_emit_block<L>(az, z, origin, sink);
     });
 }
 

@@ -37,6 +37,8 @@ struct SoASink {
 
 // One 256-point tile per CTA: with the burst L2 prefetch the input load is an L2 hit, and a deep grid lets the hardware CTA
 // scheduler balance the SMs (251 vs 256 / 258 us for 1 / 2 / 4 tiles per CTA on the 128^3 grid at lmax = 9).
+// Spinor, 16- and 32-byte store variants: ptxas takes 146 registers, i.e. ONE 256-thread CTA per SM.  Capped at 128 (two CTAs, 40-88 bytes
+// of spills) the lmax = 9 kernel is SLOWER (3.88 vs 3.77 ms on 2^22 points): the 32-byte stores of 8 warps already saturate the write stream.
 template <int KIND, int LMAX, typename T, typename TI, int VEC, bool ANGULAR>
 __global__ void __launch_bounds__(256) sh_soa_kernel(const TI* __restrict__ xyz, int64_t n, T* __restrict__ out, int coords, InputPrefetch pf) {
     constexpr int ES = elem_scalars(KIND);
@@ -66,8 +68,9 @@ constexpr int SOA_SPLIT = 2;
 
 template <int PTS, typename T = double>
 struct TileSink {
-    T* col;   // tile + this thread's point
+    T* col;   // tile + this thread's point (complex: + 2 * point)
     template <int K> __device__ __forceinline__ void put1(T v) { col[K * PTS] = v; }
+    template <int K> __device__ __forceinline__ void put2(T re, T im) { *reinterpret_cast<double2*>(col + K * 2 * PTS) = make_double2(re, im); }   // 16-byte stores, consecutive lanes: conflict-free
     template <int L> __device__ __forceinline__ void end_l() {}
     template <int L> __device__ __forceinline__ void polar(const T (&)[L + 1]) {}
 };
@@ -77,11 +80,13 @@ struct TileSink {
 // Two CTAs per SM is what the 102 KB tile allows.  fp32 (512 threads with SPLIT = 2) needs the register cap of minBlocks = 2;
 // for fp64 minBlocks stays unspecified (0): given a cap, ptxas spends registers up to it (64 -> 120 at minBlocks = 2, and 148,
 // i.e. ONE resident CTA and 0.41 instead of 0.24 ms, at minBlocks = 1).
-template <typename T, int LMAX, int WARPS, int SPLIT, bool ANGULAR>
+// KIND_COMPLEX (sh_complex): elements of 16 bytes, so 64-point tiles keep the 1 KB rows; `out` is seen as fp64 [K][2 n], box {128, K}.
+template <typename T, int LMAX, int WARPS, int SPLIT, bool ANGULAR, int KIND = KIND_REAL>
 __global__ void __launch_bounds__(32 * WARPS * SPLIT, sizeof(T) == 4 ? 2 : 0) sh_soa_tma_kernel(const T* __restrict__ xyz, int64_t n,
                                                                                                   const __grid_constant__ CUtensorMap tmap, int coords,
                                                                                                   InputPrefetch pf) {
-    constexpr int PTS = 32 * WARPS;
+    constexpr int PTS = 32 * WARPS, ES = elem_scalars(KIND);
+    static_assert(KIND == KIND_REAL || (KIND == KIND_COMPLEX && sizeof(T) == 8), "real (fp64, fp32) and complex (fp64) harmonics");
     extern __shared__ __align__(128) unsigned char smem_tile[];
     constexpr int IN_BYTES = (ANGULAR ? 2 : 3) * sizeof(T);
     prefetch_input_window(xyz, n * IN_BYTES, (int64_t)PTS * IN_BYTES, pf);
@@ -91,14 +96,17 @@ __global__ void __launch_bounds__(32 * WARPS * SPLIT, sizeof(T) == 4 ? 2 : 0) sh
     if (i < n) {
         RawPoint<T, ANGULAR> pt;
         pt.load(xyz, i);
-        TileSink<PTS, T> sink{tile + p};
+        TileSink<PTS, T> sink{tile + ES * p};
         const UnitVec u = pt.unit(coords);
-        if constexpr (SPLIT == 1) evaluate<KIND_REAL, LMAX, T>(u, sink);
+        if constexpr (SPLIT == 1) evaluate<KIND, LMAX, T>(u, sink);
         else {
             const int part = threadIdx.x / PTS;   // warp-uniform
             static_for<0, SPLIT>([&](auto pc) {
                 constexpr int PART = decltype(pc)::value;
-                if (part == PART) eval_real_part<LMAX, SPLIT, PART>((T)u.x, (T)u.y, (T)u.z, u.origin, sink);   // fp32: rounded once, after the fp64 normalization
+                if (part == PART) {
+                    if constexpr (KIND == KIND_REAL) eval_real_part<LMAX, SPLIT, PART>((T)u.x, (T)u.y, (T)u.z, u.origin, sink);   // fp32: rounded once, after the fp64 normalization
+                    else eval_complex_part<LMAX, SPLIT, PART>((T)u.x, (T)u.y, (T)u.z, u.origin, sink);
+                }
             });
         }
     }
@@ -106,7 +114,7 @@ __global__ void __launch_bounds__(32 * WARPS * SPLIT, sizeof(T) == 4 ? 2 : 0) sh
     if constexpr (WARPS * SPLIT == 1) __syncwarp();
     else __syncthreads();
     if (threadIdx.x == 0) {
-        asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%1, %2}], [%3], %4;" ::"l"(&tmap), "r"((int)base), "r"(0),
+        asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%1, %2}], [%3], %4;" ::"l"(&tmap), "r"((int)(ES * base)), "r"(0),
                      "r"(smem_u32(tile)), "l"(l2_evict_first_policy())
                      : "memory");
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
@@ -356,22 +364,22 @@ int launch_soa(const TI* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
 // SoA through the tensor unit: `out` as a 2-D tensor [K][n] of fp64 / fp32 (row pitch must be a multiple of 16 bytes: n even /
 // a multiple of 4), box {points per tile, K}, tiles of 1 KB rows (128 / 256 points).  Returns SH_ERR_ALIGNMENT when this launch
 // cannot use the path (the caller then takes the LSU-store kernels).
-template <int LMAX, bool ANGULAR = false, typename T = double>
+template <int LMAX, bool ANGULAR = false, typename T = double, int KIND = KIND_REAL>
 int launch_soa_tma(const T* xyz, int64_t n, T* out, int coords, cudaStream_t st) {
-    constexpr int K = (LMAX + 1) * (LMAX + 1);
-    constexpr int TMA_WARPS = SOA_TMA_WARPS * (int)(sizeof(double) / sizeof(T));
+    constexpr int K = (LMAX + 1) * (LMAX + 1), ES = elem_scalars(KIND);
+    constexpr int TMA_WARPS = SOA_TMA_WARPS * (int)(sizeof(double) / sizeof(T)) / ES;   // rows of 1 KB: 128 fp64, 256 fp32, 64 complex128 points
     constexpr int PTS = 32 * TMA_WARPS;
     EncodeTiledFn enc = encode_tiled();
-    if (!enc || (n * sizeof(T)) % 16 != 0 || n < PTS || n > 0x7fffff00LL || !aligned(out, 16)) return SH_ERR_ALIGNMENT;
+    if (!enc || (n * ES * sizeof(T)) % 16 != 0 || n < PTS || n * ES > 0x7fffff00LL || !aligned(out, 16)) return SH_ERR_ALIGNMENT;
     CUtensorMap tmap;
-    const cuuint64_t gdim[2] = {(cuuint64_t)n, (cuuint64_t)K};
-    const cuuint64_t gstride[1] = {(cuuint64_t)n * sizeof(T)};
-    const cuuint32_t box[2] = {PTS, (cuuint32_t)K}, estride[2] = {1, 1};
+    const cuuint64_t gdim[2] = {(cuuint64_t)n * ES, (cuuint64_t)K};
+    const cuuint64_t gstride[1] = {(cuuint64_t)n * ES * sizeof(T)};
+    const cuuint32_t box[2] = {PTS * ES, (cuuint32_t)K}, estride[2] = {1, 1};
     if (enc(&tmap, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, out, gdim, gstride, box, estride, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
             CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return SH_ERR_ALIGNMENT;
     const int64_t blocks = (n + PTS - 1) / PTS;
-    constexpr size_t smem = (size_t)K * PTS * sizeof(T);
+    constexpr size_t smem = (size_t)K * PTS * ES * sizeof(T);
     static_assert(smem <= 227 * 1024, "tile exceeds shared memory");
     auto launch = [&](auto kern, int split, SmemOptIn& opted_in) -> int {
         const int rc = ensure_dynamic_smem(kern, smem, opted_in);
@@ -381,9 +389,9 @@ int launch_soa_tma(const T* xyz, int64_t n, T* out, int coords, cudaStream_t st)
     };
     static SmemOptIn opted_in[2];
     if constexpr (LMAX >= 4) {
-        if (tuned(SH_TUNE_SOA_SPLIT, SOA_SPLIT) >= 2) return launch(sh_soa_tma_kernel<T, LMAX, TMA_WARPS, 2, ANGULAR>, 2, opted_in[1]);
+        if (tuned(SH_TUNE_SOA_SPLIT, SOA_SPLIT) >= 2) return launch(sh_soa_tma_kernel<T, LMAX, TMA_WARPS, 2, ANGULAR, KIND>, 2, opted_in[1]);
     }
-    return launch(sh_soa_tma_kernel<T, LMAX, TMA_WARPS, 1, ANGULAR>, 1, opted_in[0]);
+    return launch(sh_soa_tma_kernel<T, LMAX, TMA_WARPS, 1, ANGULAR, KIND>, 1, opted_in[0]);
 }
 
 // staging capacity per row, in scalars: whole rows for real (800 B at lmax = 9) and complex (1600 B);
@@ -451,6 +459,13 @@ int dispatch_lmax(const TI* xyz, int64_t n, T* out, int layout, int path, int co
             // one tensor-map store per 128-point tile where `out` allows it (16-byte aligned, even n)
             if (path == SH_STORE_AUTO && tuned(SH_TUNE_SOA_TMA, 0) != 1) {
                 const int rc = launch_soa_tma<LMAX>(reinterpret_cast<const double*>(xyz), n, reinterpret_cast<double*>(out), coords, st);
+                if (rc != SH_ERR_ALIGNMENT) return rc;
+            }
+        }
+        if constexpr (KIND == KIND_COMPLEX && std::is_same<T, double>::value) {
+            // one tensor store per 64-point tile where `out` allows it (16-byte aligned)
+            if (path == SH_STORE_AUTO && tuned(SH_TUNE_SOA_TMA, 0) != 1) {
+                const int rc = launch_soa_tma<LMAX, false, double, KIND_COMPLEX>(reinterpret_cast<const double*>(xyz), n, reinterpret_cast<double*>(out), coords, st);
                 if (rc != SH_ERR_ALIGNMENT) return rc;
             }
         }

@@ -140,6 +140,59 @@ def test_soa_tensor_store_and_lsu_store_paths(sh, oracle_mod, lmax):
             assert np.array_equal(got, got_lsu), (n, split)
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("lmax", [0, 3, 4, 9])
+def test_complex_soa_tensor_store_and_lsu_store_paths(sh, oracle_mod, lmax):
+    """sh_complex SoA: one TMA tensor store per 64-point tile (n >= 64, 16-byte aligned out) or per-thread 16-byte streaming stores
+    (`soa_tma` = 1, or what the alignment leaves).  Both against the oracle and against each other (bit-identical), with full tiles, a
+    ragged last tile, odd n and fewer points than one tile; one or two warps per 32-point group."""
+    rng = np.random.default_rng(400 + lmax)
+    for n in (63, 64, 65, 191, 1000, 4099):
+        pts = rng.uniform(-2, 2, (n, 3))
+        pts[0] = 0.0                     # r = 0 convention
+        pts[1] = (0.0, 0.0, 2.5)         # pole
+        want = oracle_eval(oracle_mod, "complex", pts, lmax)
+        got_tma = gpu_eval(sh, "complex", pts, lmax, "soa")
+        sh.set_tuning("soa_tma", 1)
+        try:
+            got_lsu = gpu_eval(sh, "complex", pts, lmax, "soa")
+        finally:
+            sh.set_tuning("soa_tma", 0)
+        assert max_err(got_tma, want) <= TOL64 and max_err(got_lsu, want) <= TOL64, n
+        assert np.array_equal(got_tma, got_lsu), n
+        for split in (1, 2):
+            sh.set_tuning("soa_split", split)
+            try:
+                got = gpu_eval(sh, "complex", pts, lmax, "soa")
+            finally:
+                sh.set_tuning("soa_split", 0)
+            assert np.array_equal(got, got_lsu), (n, split)
+
+
+@pytest.mark.parametrize("lmax", range(10))
+def test_real_sum_is_the_sum_of_the_harmonics(sh, oracle_mod, cube_points, lmax):
+    """sh_real_sum (the accumulate-and-never-store protocol of the paper's Table I): out[i] = sum_k R_k(point i), against the
+    oracle's values summed in long double order-independently (fsum), all three front ends, ragged sizes, specials included."""
+    import math
+    import torch
+
+    pts = cube_points[:3001]
+    want = np.array([math.fsum(row) for row in oracle_mod.real(pts, lmax)])
+    k = (lmax + 1) ** 2
+    got = sh.sh_real_sum(torch.from_numpy(pts).cuda(), lmax).cpu().numpy()
+    assert np.abs(got - want).max() <= k * 1e-14          # K values of <= 1e-14 each, far inside the 1e-12 of every single one
+    r = np.linalg.norm(pts, axis=1)
+    ok = r > 0
+    unit = pts[ok] / r[ok, None]
+    got_n = sh.sh_real_sum(torch.from_numpy(np.ascontiguousarray(unit)).cuda(), lmax, coords="normalized").cpu().numpy()
+    assert np.abs(got_n - want[ok]).max() <= k * 1e-14
+    ang = np.ascontiguousarray(np.stack([np.arccos(np.clip(unit[:, 2], -1, 1)), np.arctan2(unit[:, 1], unit[:, 0])], axis=1))
+    got_a = sh.sh_real_sum(torch.from_numpy(ang).cuda(), lmax, coords="angular").cpu().numpy()
+    want_a = np.array([math.fsum(row) for row in oracle_mod.real_angular(ang, lmax)])   # the oracle's angular core at the same angles
+    assert np.abs(got_a - want_a).max() <= k * 1e-14
+    assert sh.sh_real_sum(torch.empty((0, 3), dtype=torch.float64, device="cuda"), lmax).numel() == 0
+
+
 @pytest.mark.parametrize("kind", ["real", "complex", "spinor"])
 @pytest.mark.parametrize("layout", ["soa", "aos"])
 def test_misaligned_out_and_odd_n_fall_back(sh, oracle_mod, kind, layout):
