@@ -187,6 +187,20 @@ def ceilings(dev, sampler_index=None):
     }
 
 
+def ncu_fp64_executed(kernel_key: str):
+    """FP64 thread-instructions executed per launch of a kernel family on the 128^3 grid (profiles/ncu_fp64_instr.csv, from the committed
+    `ncu --set full` captures), or None: what the kernel really issues, next to the algorithmic count `roofline.frac` is built on."""
+    try:
+        import csv
+
+        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "ncu_fp64_instr.csv"))):
+            if row["kernel"] == kernel_key:
+                return float(row["fp64_thread_instr_per_launch"])
+    except Exception:
+        pass
+    return None
+
+
 def hbm_roofline(kernel, alg_bytes, written_bytes, ms, peak, peak_src, ceil, pattern, traffic_key=None):
     """`roofline` block of an HBM-bound launch: achieved = algorithmic bytes (in + out) per launch / average launch time against
     the driver-measured copy peak, plus the written bytes against the write-only fill ceiling of the kernel's own store pattern."""
@@ -487,8 +501,14 @@ def projector_cases(sh, dev, timed, timed_graph, want, ceil=None):
                 "read_GBps": n * (24 + 8 * nvec) / ms / 1e6,
                 "roofline": {"bound": "alu", "unit": "G FP64 lane-instr/s", "achieved": n * fp64_per_point / ms / 1e6,
                              "peak": peak_ginstr, "frac": n * fp64_per_point / ms / 1e6 / peak_ginstr, "peak_source": peak_src,
-                             "peak_nominal": nominal_ginstr, "fp64_instr_per_point": fp64_per_point},
+                             "peak_nominal": nominal_ginstr, "fp64_instr_per_point": fp64_per_point,
+                             "what": "algorithmic FP64 work of the method (factorized forms) per second over the measured FP64 pipe peak"},
             }
+            executed = ncu_fp64_executed(f"project_nv{nvec}") if n == 128 ** 3 else None
+            if executed:   # the default Horner / recurrence forms issue fewer FP64 instructions than the algorithmic count
+                res[f"project nvec={nvec} {name}"]["roofline"].update({
+                    "fp64_instr_per_point_executed": executed / n, "frac_executed": executed / ms / 1e6 / peak_ginstr,
+                    "executed_source": "profiles/ncu_fp64_instr.csv (ncu smsp__sass_thread_inst_executed_op_d*_pred_on of the same launch)"})
             if n < (1 << 18):
                 res[f"project nvec={nvec} {name}"].update({"ms": ms_py, "ms_in_cuda_graph": ms})
             else:
@@ -511,7 +531,9 @@ def projector_cases(sh, dev, timed, timed_graph, want, ceil=None):
 # compiled for the store kernels (cuobjdump: 94 at lmax = 3, 566 at lmax = 9), plus the radial position (sqrt, ~12) and the
 # table interpolation (3 per channel: 8 / 10 channels); DESIGN.md section 6.  Keys = lmax.
 PROJECT_FP64_PER_POINT = {3: 94 + 12 + 24, 9: 566 + 12 + 30}
-REAL_L9_FP64_PER_POINT = 566   # a2-a5 at lmax = 9 in the factorized forms (the store kernels' SASS count)
+REAL_L9_FP64_PER_POINT = 538   # a2-a5 at lmax = 9 in the factorized forms, one warp per point group: FP64 thread-instructions EXECUTED per point
+                               # (ncu smsp__sass_thread_inst_executed_op_d*_pred_on of sh_real AoS, profiles/ncu_fp64_instr.csv; the static SASS count, both
+                               # branches of the range scaling included, is 566-575)
 
 
 def run_ours(args):
