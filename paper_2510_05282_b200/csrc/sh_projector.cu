@@ -313,17 +313,19 @@ __global__ void __launch_bounds__(128, PROJ_SEG_CTAS) sh_project_seg_kernel(cons
 //
 //   one persistent CTA per SM = NPW producer warps + NCW consumer warps around a ring of tile slots in shared memory
 //   (slot = vals[ncols][32] + wts[NV][32] doubles; mbarrier full/empty pair per slot).
-//   PRODUCERS: SPLIT warps share one 32-point tile (lane i = point i; warp `part` evaluates the l-blocks of block_part, a2/a3
-//     repeated) and stage beta_col = f_p(r) R_l^m at vals[col][lane] (conflict-free 8-byte stores); the tile's weights go to
-//     wts[v][lane].  The radial values of a warp's own channel slots are fetched up front (independent table loads overlap)
-//     and parked in the first column cell of each channel until the block is produced.
+//   PRODUCERS: SPLIT warps per 32-point tile (lane i = point i; SPLIT = 1 in both shipped shapes: one warp evaluates the whole tile.
+//     With SPLIT > 1 warp `part` evaluates the l-blocks of block_part and a2/a3 are repeated) stage beta_col = f_p(r) R_l^m at
+//     vals[col][lane] (conflict-free 8-byte stores); the tile's weights go to wts[v][lane].  The radial values of a warp's own
+//     channel slots are fetched up front (independent table loads overlap) and parked in the first column cell of each channel
+//     until the block is produced.
 //   CONSUMERS: every consumer warp visits every tile, but owns only some columns: a lane keeps acc[v][j] for its point
 //     position and its columns IN REGISTERS across all tiles of the CTA (acc += wts[v][lane] * vals[col][lane]: one 8-byte
 //     conflict-free load per NV FMAs, no broadcast, no transpose, every lane busy), and the cross-lane sum is taken once,
 //     at the end, by a butterfly.  The accumulators are what bounds the shape: NV x ncols x 32 lanes doubles per CTA
 //     (NV = 4, 104 columns: 26.6 K of the SM's 64 K registers), hence separate consumer warps that never evaluate a
-//     polynomial, and for NV = 8 lane GROUPS: G groups of 32/G lanes own different columns and take G points each per tile
-//     (group g reads the point quarters in the rotated order (k + g) % G, so the G groups hit different banks).
+//     polynomial, and lane GROUPS: G groups of 32/G lanes own different columns and take G points each per tile (group g
+//     reads the point quarters in the rotated order (k + g) % G, so the G groups hit different banks), which divides the
+//     accumulators per lane by G.
 //   The consumers' FMAs are independent and fill the FP64-pipe bubbles of the producers' dependent polynomial chains.
 // Tiles are dealt round-robin to the CTAs (static: the summation order is fixed, results are reproducible); idle lanes of a
 // ragged last tile stage the point (0, 0, 1) with weight 0.  One row of `partial` [cta][nvec][ncols] per CTA, then
@@ -331,11 +333,13 @@ __global__ void __launch_bounds__(128, PROJ_SEG_CTAS) sh_project_seg_kernel(cons
 
 template <int NV> struct ProjCfg;
 //                                   producer warps, warps per tile, consumer warps, lane groups per consumer warp
-// 20 warps = 640 threads leave 96 registers per thread: the producers' polynomial code needs them (at 80, with 16 + 8 warps, it spills
-// and a tile takes 7200 instead of 5700 cycles), and two consumer warps per scheduler get the issue share their FMAs need (with one,
-// the consumers, not the producers, set the time: 0.268 vs 0.247 ms for four vectors on the 128^3 grid).
-template <> struct ProjCfg<4> { static constexpr int NPW = 12, SPLIT = 2, NCW = 8, G = 2; };
-template <> struct ProjCfg<8> { static constexpr int NPW = 10, SPLIT = 2, NCW = 10, G = 4; };   // eight vectors: 0.356 ms with 10 + 10, 0.452 with 12 + 8
+// One producer warp per tile (SPLIT = 1): nothing of a2/a3 or the radial look-up is repeated, and with 12 or 16 warps per CTA the
+// compiler has 168 / 128 registers to overlap the polynomial chains of an l-block (a whole tile in ~7300 cycles, against 2 x 5700 for two
+// warps sharing it at 96 registers).  The ring holds 8 tiles at 100 columns, so 8 producers; the consumer warps follow from the FMA load:
+// four (G = 4: 32 accumulator registers) for up to four vectors, eight for eight.
+template <> struct ProjCfg<4> { static constexpr int NPW = 8, SPLIT = 1, NCW = 4, G = 4; };
+template <> struct ProjCfg<8> { static constexpr int NPW = 8, SPLIT = 1, NCW = 8, G = 4; };
+static_assert(ProjCfg<4>::SPLIT == ProjCfg<8>::SPLIT, "run_project builds one per-part channel list for both");
 
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
@@ -724,7 +728,6 @@ template <int LMAX, int NV>
 int launch_project_ring(const double* xyz, int64_t n, const double* radial, const ProjPlan& plan, const double* w, int nvec, double* partial,
                         int64_t* rows, cudaStream_t st) {
     using Cfg = ProjCfg<NV>;
-    static_assert(Cfg::SPLIT == 2, "fill_parts<2> in run_project");
     // ring of tile slots: as many as fit (at most PROJ_RING_MAX), then the 2 x PROJ_RING_MAX mbarriers
     const size_t slot_bytes = (size_t)(plan.ncols + NV) * 32 * sizeof(double);
     int nring = (int)(((size_t)227 * 1024 - 2 * PROJ_RING_MAX * sizeof(uint64_t)) / slot_bytes);
@@ -780,7 +783,7 @@ int run_project(const double* xyz, int64_t n, int nproj, const int* proj_l, cons
         while (p1 < nproj && cols + 2 * proj_l[p1] + 1 <= PROJ_MAX_COLS) cols += 2 * proj_l[p1++] + 1;
         ProjPlan plan;
         const int lmax = make_plan(proj_l, p0, p1, nr, dr, plan);
-        fill_parts<2>(proj_l, plan);   // every ProjCfg uses two warps per tile
+        fill_parts<ProjCfg<4>::SPLIT>(proj_l, plan);
         for (int v0 = 0; v0 < nvec; v0 += PROJ_NV) {
             const int nv = nvec - v0 < PROJ_NV ? nvec - v0 : PROJ_NV;
             switch (lmax) {

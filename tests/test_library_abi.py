@@ -73,6 +73,12 @@ def test_argument_validation_without_gpu(lib):
         assert fn(p, 4, 20, p, 1 | (2 << 8), None) == -4  # nor the bulk store path
         assert fn(None, 4, 20, p, 1, None) == -1 and fn(None, 0, 20, None, 1, None) == 0
         assert fn(p, 4, 20, p + 4, 1, None) == -5
+    # sh_real_sum: `coords` is one SH_COORDS_* value, no layout bits
+    f = lib.sh_real_sum
+    assert f(p, -1, 3, p, 0, None) == -2 and f(p, 4, 10, p, 0, None) == -3 and f(p, 4, -1, p, 0, None) == -3
+    assert f(p, 4, 3, p, 1, None) == -4 and f(p, 4, 3, p, 3 << 16, None) == -4          # a layout bit, an unknown front end
+    assert f(None, 4, 3, p, 0, None) == -1 and f(p, 4, 3, None, 1 << 16, None) == -1
+    assert f(p, 4, 3, p + 4, 2 << 16, None) == -5 and f(None, 0, 3, None, 0, None) == 0
     for fn in (lib.sh_real_host, lib.sh_complex_host, lib.sh_spinor_host, lib.sh_real_f32_host):
         assert fn(p, -1, 3, p, 0) == -2 and fn(p, 1, 11, p, 0) == -3 and fn(None, 0, 3, None, 1) == 0
     # fused projector consumer: every argument is checked on the host
