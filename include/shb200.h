@@ -182,8 +182,8 @@ enum {
     SH_TUNE_PREFETCH_WINDOW_POINTS = 0, /* points per burst of the L2 input prefetch (default 262144); 1 = prefetch off */
     SH_TUNE_PROJ_AOS_MODE = 1,      /* sh_projectors AoS copy-out: 1 = warp copy, 2 = one bulk copy per row, 3 = one per tile (when possible) */
     SH_TUNE_SOA_TMA = 2,            /* SoA through TMA tensor stores (sh_real, sh_real_f32, sh_complex; tiles staged in shared memory): 0 = when possible (default), 1 = never (per-thread streaming stores) */
-    SH_TUNE_PROJECT_FORM = 3,       /* sh_project polynomials: 0 = default; 1 = Horner in z^2 for the polar factors and (x + iy)^m by
-                                       recurrence; 2 = the factorized root-pair forms of every other call */
+    SH_TUNE_PROJECT_FORM = 3,       /* sh_project polynomials: 0 or 1 = Horner in z^2 for the polar factors and (x + iy)^m by recurrence (the
+                                       default of this one FP64-bound call); 2 = the factorized root-pair forms of every other call */
     SH_TUNE_PROJ_AOS_SPLIT = 4,     /* sh_projectors AoS, lmax >= 4: warps that share one 32-point tile, each evaluating part of the l-blocks: 1, 2 (default) or 4 */
     SH_TUNE_SOA_SPLIT = 5,          /* sh_real / sh_real_f32 SoA tensor-store path, lmax >= 4: warps that share a 32-point group of the tile, each evaluating part of the l-blocks: 1 or 2 (default) */
     SH_TUNE_COUNT = 6

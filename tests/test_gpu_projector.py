@@ -110,9 +110,10 @@ def test_every_lmax_unsorted_channels_and_ragged_sizes(sh, oracle_mod, lmax):
         for layout, mis in (("soa", 0), ("aos", 0), ("aos", 1), ("soa", 1)):
             got = gpu_projectors(sh, pts, proj_l, tab, dr, layout, misalign=mis)
             assert np.abs(got - want).max() <= TOL * max(1.0, np.abs(tab).max()), (n, layout, mis)
-        w = rng.standard_normal((2, n))
-        coeff, abs_sum = oracle_mod.project(pts, proj_l, tab, dr, w)
-        check_project(gpu_project(sh, pts, proj_l, tab, dr, w), coeff, abs_sum)
+        for nvec in (1, 2, 5):   # segment kernel; ring kernel with four- and eight-vector consumers
+            w = rng.standard_normal((nvec, n))
+            coeff, abs_sum = oracle_mod.project(pts, proj_l, tab, dr, w)
+            check_project(gpu_project(sh, pts, proj_l, tab, dr, w), coeff, abs_sum)
 
 
 @pytest.mark.parametrize("proj_l", [[2], [0, 1, 3], [1, 1], [0, 2, 1, 3], [9, 9, 9, 4, 0], [0, 1, 2, 3, 4, 5, 6, 7, 8, 9], [5, 4, 4, 7], [9] * 11, [9] * 12])
