@@ -449,11 +449,13 @@ __global__ void __launch_bounds__(32 * (ProjCfg<NV>::NPW + ProjCfg<NV>::NCW), 1)
         // point index of this lane in the stream's current tile; the stream advances by STREAMS * gridDim.x tiles
         int64_t i = (((int64_t)blockIdx.x + (int64_t)stream * gridDim.x) << 5) + lane;
         const int64_t istep = ((int64_t)STREAMS * gridDim.x) << 5;
+        // The next tile's point is loaded a whole tile ahead and NOT touched until then: a select on the loaded value right behind the
+        // load would make the warp wait for it at once (it did: 14 % of the producers' time).  Idle lanes of a ragged last tile read the
+        // last point and are replaced by a harmless one (weights 0) where the values are used.  Streaming loads (evict-first): what
+        // should stay in the small L1 next to 213 KB of ring is the radial table.
         auto load_point = [&](int64_t ip, double& x, double& y, double& z) {
-            const bool ok = ip < n;   // idle lane of the ragged last tile: a harmless point (its weights are 0)
-            const double* p = xyz + 3 * (ok ? ip : 0);
-            const double a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
-            x = ok ? a : 0.0; y = ok ? b : 0.0; z = ok ? c : 1.0;
+            const double* p = xyz + 3 * (ip < n ? ip : n - 1);
+            x = __ldcs(p); y = __ldcs(p + 1); z = __ldcs(p + 2);
         };
         double x = 0.0, y = 0.0, z = 1.0, nx = 0.0, ny = 0.0, nz = 1.0;
         int64_t seq = stream;
@@ -461,17 +463,20 @@ __global__ void __launch_bounds__(32 * (ProjCfg<NV>::NPW + ProjCfg<NV>::NCW), 1)
         int slot = stream % nring, use = stream / nring;
         for (; seq < my_tiles; seq += STREAMS, i += istep) {
             if (seq + STREAMS < my_tiles) load_point(i + istep, nx, ny, nz);
-            // the tile's weights: vector v is fetched by warp part v % SPLIT
+            // the tile's weights: vector v is fetched by warp part v % SPLIT; masked where they are stored
             constexpr int WPP = (NV + SPLIT - 1) / SPLIT;
             double wv[WPP];
+            const bool ok = i < n;
+            const int64_t iw = ok ? i : n - 1;
             static_for<0, WPP>([&](auto kc) {
                 const int v = part + decltype(kc)::value * SPLIT;
-                wv[decltype(kc)::value] = (v < nvec && i < n) ? __ldg(w + (int64_t)v * n + i) : 0.0;
+                wv[decltype(kc)::value] = __ldcs(w + (int64_t)(v < nvec ? v : 0) * n + iw);
             });
+            if (!ok) { x = 0.0; y = 0.0; z = 1.0; }
             if (use > 0) mbar_wait(empty + slot, (use - 1) & 1);   // the consumers have released the slot's previous tile
             double* sv = ring + (size_t)slot * slot_doubles + lane;
             const RadialPos pos(x, y, z, plan);
-#pragma unroll 4
+#pragma unroll 8   // eight channels' table loads in flight (4: 0.230 ms, 8: 0.228, 16: 0.279 for four vectors on the 128^3 grid)
             for (int k = ps0; k < ps1; ++k) {
                 const int s = plan.part_slots[k];
                 sv[plan.col[s] * 32] = pos.f_row(radial + plan.row[s]);
@@ -484,7 +489,7 @@ __global__ void __launch_bounds__(32 * (ProjCfg<NV>::NPW + ProjCfg<NV>::NCW), 1)
             });
             static_for<0, WPP>([&](auto kc) {
                 const int v = part + decltype(kc)::value * SPLIT;
-                if (v < NV) sv[(ncols + v) * 32] = wv[decltype(kc)::value];
+                if (v < NV) sv[(ncols + v) * 32] = (ok && v < nvec) ? wv[decltype(kc)::value] : 0.0;
             });
             __syncwarp();
             if (lane == 0) mbar_arrive(full + slot);
