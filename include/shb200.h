@@ -89,7 +89,8 @@ enum {
     SH_ERR_LAYOUT = -4,    /* unknown layout, store-path or front-end bits */
     SH_ERR_ALIGNMENT = -5, /* out not aligned to its element type, or requested store path not possible */
     SH_ERR_CUDA = -6,      /* CUDA launch / copy error; text via sh_last_cuda_error() */
-    SH_ERR_PROJECTOR = -7  /* sh_projectors / sh_project: nproj, proj_l, nr, dr, nvec or the workspace size is invalid */
+    SH_ERR_PROJECTOR = -7, /* sh_projectors / sh_project: nproj, proj_l, nr, dr, nvec or the workspace size is invalid */
+    SH_ERR_SCRATCH = -8    /* sh_project_static: the request needs more scratch than the library's static device array holds */
 };
 
 /* Real harmonics R_l^m (Eq. 6), fp64.  out: K doubles per point. */
@@ -150,6 +151,21 @@ int sh_projectors(const double* xyz, int64_t n, int nproj, const int* proj_l, co
                   double* out, int layout, void* stream);
 int sh_project(const double* xyz, int64_t n, int nproj, const int* proj_l, const double* radial, int nr, double dr,
                const double* w, int nvec, double* coeff, void* workspace, int64_t workspace_bytes, void* stream);
+
+/* sh_project without any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it): the same computation and the same kernels as sh_project, bit-identical results, but the per-CTA
+ * partial sums live in a static device array inside the library instead of a caller-provided workspace.  The caller still passes
+ * every input and the output `coeff` (DEVICE pointers; `proj_l` HOST).  The call allocates nothing and frees nothing.
+ *   Limit: the array holds sh_project_static_bytes() = 2 MiB on every GPU that loads the library (until the process exits).  A request
+ *   with sh_project_workspace_bytes(ncols, nvec) above that returns SH_ERR_SCRATCH and launches nothing; on a 148-SM B200 this means
+ *   min(nvec, 8) x min(ncols, 104) <= 442: any number of columns with up to 4 weight vectors, up to 55 columns with 5 to 8 (split a
+ *   wider request into calls of 4 vectors, or use sh_project with your own workspace).
+ *   Sharing: every call on a device uses the SAME array.  Calls ordered on one stream are safe (nothing in the array has to start at
+ *   zero or survives a call); calls that OVERLAP on the GPU -- different streams, concurrently replayed graphs -- race and give
+ *   wrong coefficients.  Use sh_project with separate workspaces for those. */
+int sh_project_static(const double* xyz, int64_t n, int nproj, const int* proj_l, const double* radial, int nr, double dr,
+                      const double* w, int nvec, double* coeff, void* stream);
+int64_t sh_project_static_bytes(void);   /* size of the static scratch array: 2097152 */
 
 /* Host-buffer entry points: same results, `xyz` and `out` are HOST pointers (pinned memory gives full
  * PCIe speed; pageable memory works).  The call copies chunks host->device, runs the kernels and copies

@@ -21,6 +21,8 @@ from .binding import (  # noqa: F401
     sh_complex,
     sh_complex_ext,
     sh_project,
+    sh_project_static,
+    project_static_bytes,
     sh_projectors,
     sh_real,
     sh_real_ext,

@@ -84,6 +84,9 @@ def load() -> ctypes.CDLL:
         lib.sh_projectors.restype = ci
         lib.sh_project.argtypes = [vp, i64, ci, ip, vp, ci, ctypes.c_double, vp, ci, vp, vp, i64, vp]
         lib.sh_project.restype = ci
+        lib.sh_project_static.argtypes = [vp, i64, ci, ip, vp, ci, ctypes.c_double, vp, ci, vp, vp]
+        lib.sh_project_static.restype = ci
+        lib.sh_project_static_bytes.restype = i64
         _lib = lib
     return _lib
 
@@ -336,4 +339,32 @@ def sh_project(xyz, proj_l, radial, dr, w, coeff=None, workspace=None, stream=No
                                coeff.data_ptr(), workspace.data_ptr(), workspace.numel() * workspace.element_size(), s)
     if rc != 0:
         raise ShError(rc, "sh_project")
+    return coeff
+
+
+def project_static_bytes() -> int:
+    """Size of the static scratch array sh_project_static works in (2 MiB)."""
+    return int(load().sh_project_static_bytes())
+
+
+def sh_project_static(xyz, proj_l, radial, dr, w, coeff, stream=None):
+    """sh_project without any allocation (include/shb200.h "sh_project_static"): the per-CTA partial sums live in a static device
+    array inside the library, so `coeff` [nvec][ncols] must be given and nothing is allocated here either.  Raises ShError with
+    code -8 (SH_ERR_SCRATCH) when the request needs more than project_static_bytes().  Calls that overlap on the GPU race."""
+    import torch
+
+    a, nproj = _proj_l_array(proj_l)
+    _check_proj_inputs(xyz, radial, nproj)
+    n, ncols = xyz.shape[0], projector_count(proj_l)
+    if not (w.is_cuda and w.dtype == torch.float64 and w.is_contiguous() and w.dim() == 2 and w.shape[1] == n):
+        raise ValueError("w must be a contiguous CUDA tensor [nvec][n] of float64")
+    nvec = w.shape[0]
+    if not (coeff.is_cuda and coeff.dtype == torch.float64 and coeff.is_contiguous() and coeff.numel() == nvec * ncols):
+        raise ValueError(f"coeff must be a contiguous CUDA float64 tensor with {nvec * ncols} elements")
+    s = torch.cuda.current_stream(xyz.device).cuda_stream if stream is None else int(stream)
+    with torch.cuda.device(xyz.device):
+        rc = load().sh_project_static(xyz.data_ptr(), n, nproj, a, radial.data_ptr(), radial.shape[1], float(dr), w.data_ptr(), nvec,
+                                      coeff.data_ptr(), s)
+    if rc != 0:
+        raise ShError(rc, "sh_project_static")
     return coeff

@@ -97,6 +97,7 @@ const char* sh_strerror(int code) {
         case SH_ERR_ALIGNMENT: return "pointer not aligned to its element type, or requested store path impossible for this alignment";
         case SH_ERR_CUDA: return "CUDA error (see sh_last_cuda_error)";
         case SH_ERR_PROJECTOR: return "bad projector arguments (nproj, proj_l, nr, dr, nvec or workspace size)";
+        case SH_ERR_SCRATCH: return "sh_project_static: the request needs more than the 2 MiB static scratch array (see sh_project_static_bytes; use sh_project with a workspace)";
     }
     return "unknown error code";
 }

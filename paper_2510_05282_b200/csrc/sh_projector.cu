@@ -804,6 +804,59 @@ int run_project(const double* xyz, int64_t n, int nproj, const int* proj_l, cons
     return SH_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// sh_project_static: sh_project for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid
+// cudaMalloc).  The per-CTA partial sums that sh_project keeps in the caller's `workspace` live in this file-scope device array
+// instead: PROJ_STATIC_BYTES = 2 MiB, held by every GPU that loads the library until the process exits.  A request whose
+// sh_project_workspace_bytes(ncols, nvec) exceeds it is refused with SH_ERR_SCRATCH (on a 148-SM B200: min(nvec, 8) x min(ncols, 104)
+// <= 442, i.e. any width with up to 4 weight vectors, up to 55 columns with 5 to 8; more vectors or columns per call run as several
+// passes over the same array, so only these two capped factors count).
+// In HOST code the array's name is a host-side stand-in, not a device address (a kernel handed `g_project_scratch` itself would fault,
+// or, where the GPU can reach host memory, silently use the wrong memory): the device address comes from cudaGetSymbolAddress, asked
+// once per device with that device current, and is what the kernels get.
+// Nothing has to start at zero: every row of partial sums the ordered reduction reads was written by a kernel of the SAME call before
+// it (each CTA stores, not accumulates, its full row), so the contents a previous call left behind are never read.  All calls on a
+// device share the one array: calls that overlap on the GPU (different streams, or graphs replayed concurrently) race.
+constexpr size_t PROJ_STATIC_BYTES = (size_t)2 << 20;
+static __device__ __align__(256) double g_project_scratch[PROJ_STATIC_BYTES / sizeof(double)];
+
+// device address of g_project_scratch on the CURRENT device (cached per device; racing threads resolve the same value)
+int project_scratch_address(double** out) {
+    static std::atomic<double*> cache[64];   // static storage: null-initialised
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    double* ptr = dev < 64 ? cache[dev].load(std::memory_order_acquire) : nullptr;
+    if (!ptr) {
+        e = cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_project_scratch);
+        if (e != cudaSuccess) return cuda_fail(e);
+        if (!ptr) return SH_ERR_CUDA;
+        if (dev < 64) cache[dev].store(ptr, std::memory_order_release);
+    }
+    *out = ptr;
+    return SH_OK;
+}
+
+int run_project_static(const double* xyz, int64_t n, int nproj, const int* proj_l, const double* radial, int nr, double dr, const double* w,
+                       int nvec, double* coeff, void* stream) {
+    // the argument checks of sh_project that need no workspace come first, so that a bad call is reported as what it is
+    const int rc = check_projector_args(xyz, n, nproj, proj_l, radial, nr, dr);
+    if (rc != SH_OK) return rc;
+    if (nvec < 0) return SH_ERR_PROJECTOR;
+    const int ncols = projector_count(nproj, proj_l);
+    if (nvec == 0 || ncols == 0) return SH_OK;
+    const int64_t need = project_workspace_bytes(ncols, nvec);
+    if (need < 0 || need > (int64_t)PROJ_STATIC_BYTES) return SH_ERR_SCRATCH;
+    double* scratch = nullptr;
+    if (n > 0) {   // the empty sum launches nothing that reads the scratch
+        const int rs = project_scratch_address(&scratch);
+        if (rs != SH_OK) return rs;
+    }
+    // the same code path as sh_project from here on, with the static array as its workspace: no cudaMalloc, cudaFree or allocating
+    // library routine anywhere below (plans live on the host stack, kernels take them by value)
+    return run_project(xyz, n, nproj, proj_l, radial, nr, dr, w, nvec, coeff, scratch, n > 0 ? (int64_t)PROJ_STATIC_BYTES : 0, stream);
+}
+
 
 }  // namespace shb200
 
@@ -821,5 +874,10 @@ int sh_project(const double* xyz, int64_t n, int nproj, const int* proj_l, const
                int nvec, double* coeff, void* workspace, int64_t workspace_bytes, void* stream) {
     return run_project(xyz, n, nproj, proj_l, radial, nr, dr, w, nvec, coeff, workspace, workspace_bytes, stream);
 }
+int sh_project_static(const double* xyz, int64_t n, int nproj, const int* proj_l, const double* radial, int nr, double dr, const double* w,
+                      int nvec, double* coeff, void* stream) {
+    return run_project_static(xyz, n, nproj, proj_l, radial, nr, dr, w, nvec, coeff, stream);
+}
+int64_t sh_project_static_bytes(void) { return (int64_t)PROJ_STATIC_BYTES; }
 
 }  // extern "C"
