@@ -202,7 +202,8 @@ enum {
                                        default of this one FP64-bound call); 2 = the factorized root-pair forms of every other call */
     SH_TUNE_PROJ_AOS_SPLIT = 4,     /* sh_projectors AoS, lmax >= 4: warps that share one 32-point tile, each evaluating part of the l-blocks: 1, 2 (default) or 4 */
     SH_TUNE_SOA_SPLIT = 5,          /* sh_real / sh_real_f32 SoA tensor-store path, lmax >= 4: warps that share a 32-point group of the tile, each evaluating part of the l-blocks: 1 or 2 (default) */
-    SH_TUNE_COUNT = 6
+    SH_TUNE_PROJ_AOS_PAIRS = 6,     /* sh_projectors AoS staging: 0 = 16-byte stores where the rows allow (default), 1 = 8-byte stores always */
+    SH_TUNE_COUNT = 7
 };
 int sh_set_tuning(int knob, int value);
 

@@ -116,7 +116,7 @@ def index_spinor(l: int, twoj: int, twomj: int) -> int:
     return load().sh_index_spinor(l, twoj, twomj)
 
 
-TUNE = {"prefetch_window_points": 0, "proj_aos_mode": 1, "soa_tma": 2, "project_form": 3, "proj_aos_split": 4, "soa_split": 5}
+TUNE = {"prefetch_window_points": 0, "proj_aos_mode": 1, "soa_tma": 2, "project_form": 3, "proj_aos_split": 4, "soa_split": 5, "proj_aos_pairs": 6}
 
 
 def set_tuning(knob, value: int) -> None:

@@ -122,6 +122,12 @@ __global__ void __launch_bounds__(256) sh_proj_soa_kernel(const double* __restri
 //   PROJ_AOS_PLAIN: pitch odd, the CTA copies the tile out with coalesced streaming stores (any alignment, any width).
 // A ragged last tile is always copied out by the CTA; its idle lanes evaluate the last point.
 constexpr int PROJ_AOS_PLAIN = 0, PROJ_AOS_ROWBULK = 1, PROJ_AOS_TILEBULK = 2;
+// PAIRS (rows of an even number of doubles: every row keeps 16-byte alignment): the 2l + 1 values of a channel go out as l 16-byte
+// stores and one 8-byte store, from an even or an odd start column (warp-uniform branch).  With dense 800-byte rows the 32 lanes of an
+// 8-byte staging store land on 4 bank pairs -- 8 wavefronts instead of 2, ~800 per tile, and ncu showed the shared-memory pipe (7.6-way
+// conflicts on 7.2 M store requests), not the store stream, bounding this kernel; a 16-byte store of the same lanes takes 8 wavefronts
+// for twice the data: 0.258 -> 0.237 ms on the 128^3 grid with 100 columns, the rate of sh_real AoS.
+template <bool PAIRS>
 struct ProjRowSink {
     double* row;
     const double* fs;   // this lane's radial values: fs[slot*32]
@@ -132,13 +138,28 @@ struct ProjRowSink {
 #pragma unroll 1
         for (int s = plan.first[L]; s < plan.first[L + 1]; ++s) {
             const double f = fs[s * 32];
-            double* q = row + plan.col[s];
-            static_for<0, 2 * L + 1>([&](auto mc) { q[decltype(mc)::value] = f * blk[decltype(mc)::value]; });
+            const int c = plan.col[s];
+            double* q = row + c;
+            if constexpr (!PAIRS || L == 0) {
+                static_for<0, 2 * L + 1>([&](auto mc) { q[decltype(mc)::value] = f * blk[decltype(mc)::value]; });
+            } else if ((c & 1) == 0) {
+                static_for<0, L>([&](auto jc) {
+                    constexpr int J = 2 * decltype(jc)::value;
+                    *reinterpret_cast<double2*>(q + J) = make_double2(f * blk[J], f * blk[J + 1]);
+                });
+                q[2 * L] = f * blk[2 * L];
+            } else {
+                q[0] = f * blk[0];
+                static_for<0, L>([&](auto jc) {
+                    constexpr int J = 1 + 2 * decltype(jc)::value;
+                    *reinterpret_cast<double2*>(q + J) = make_double2(f * blk[J], f * blk[J + 1]);
+                });
+            }
         }
     }
 };
 
-template <int LMAX, int SPLIT>
+template <int LMAX, int SPLIT, bool PAIRS>
 __global__ void __launch_bounds__(32 * SPLIT) sh_proj_aos_kernel(const double* __restrict__ xyz, int64_t n, const double* __restrict__ radial,
                                                                   const __grid_constant__ ProjPlan plan, double* __restrict__ out, int pitch, int mode,
                                                                   InputPrefetch pf) {
@@ -161,7 +182,7 @@ __global__ void __launch_bounds__(32 * SPLIT) sh_proj_aos_kernel(const double* _
     if constexpr (SPLIT > 1) __syncthreads();
     else __syncwarp();
     const UnitVec u = pt.unit(SH_COORDS_CARTESIAN);
-    ProjRowSink sink{tile + lane * pitch, fs + lane, plan};
+    ProjRowSink<PAIRS> sink{tile + lane * pitch, fs + lane, plan};
     static_for<0, SPLIT>([&](auto pc) {
         constexpr int PART = decltype(pc)::value;
         if (warp == PART) eval_projector_blocks<LMAX, false, SPLIT, PART>(u, plan, sink);
@@ -596,13 +617,17 @@ constexpr int PROJ_AOS_SPLIT = 2;
 template <int LMAX, int SPLIT>
 int launch_proj_aos_split(const double* xyz, int64_t n, const double* radial, const ProjPlan& plan, double* out, int pitch, int mode, size_t smem,
                           cudaStream_t st) {
-    auto kern = sh_proj_aos_kernel<LMAX, SPLIT>;
-    static SmemOptIn opted_in;   // the opt-in limit only ever grows
-    if (const int rc = ensure_dynamic_smem(kern, smem, opted_in); rc != SH_OK) return rc;
     const int64_t ntiles = (n + 31) / 32;
     if (ntiles > 0x7fffffffLL) return SH_ERR_COUNT;
-    kern<<<(unsigned)ntiles, 32 * SPLIT, smem, st>>>(xyz, n, radial, plan, out, pitch, mode, prefetch_plan(n, 32));
-    return launch_status();
+    auto launch = [&](auto kern, SmemOptIn& opted_in) -> int {
+        if (const int rc = ensure_dynamic_smem(kern, smem, opted_in); rc != SH_OK) return rc;
+        kern<<<(unsigned)ntiles, 32 * SPLIT, smem, st>>>(xyz, n, radial, plan, out, pitch, mode, prefetch_plan(n, 32));
+        return launch_status();
+    };
+    static SmemOptIn opted_in[2];   // the opt-in limit only ever grows
+    // 16-byte staging stores where every row keeps 16-byte alignment (even pitch; the staging tile itself is 16-byte aligned)
+    if (pitch % 2 == 0 && tuned(SH_TUNE_PROJ_AOS_PAIRS, 0) != 1) return launch(sh_proj_aos_kernel<LMAX, SPLIT, true>, opted_in[1]);
+    return launch(sh_proj_aos_kernel<LMAX, SPLIT, false>, opted_in[0]);
 }
 
 template <int LMAX>

@@ -133,14 +133,21 @@ def test_aos_store_modes(sh, oracle_mod, proj_l):
         for mis in (0, 1, 2):
             for mode in (0, 1, 2, 3):   # automatic, then each copy-out forced (where it applies)
                 for split in (0, 1, 2, 4):   # warps sharing a tile (lmax >= 4): default, then each forced
-                    sh.set_tuning("proj_aos_mode", mode)
-                    sh.set_tuning("proj_aos_split", split)
-                    try:
-                        got = gpu_projectors(sh, pts, proj_l, tab, dr, "aos", misalign=mis)
-                    finally:
-                        sh.set_tuning("proj_aos_mode", 0)
-                        sh.set_tuning("proj_aos_split", 0)
-                    assert np.abs(got - want).max() <= TOL * max(1.0, np.abs(tab).max()), (n, mis, mode, split)
+                    ref = None
+                    for pairs in ((0, 1) if split in (0, 1) else (0,)):   # 16-byte staging stores where the rows allow (default), or 8-byte always
+                        sh.set_tuning("proj_aos_mode", mode)
+                        sh.set_tuning("proj_aos_split", split)
+                        sh.set_tuning("proj_aos_pairs", pairs)
+                        try:
+                            got = gpu_projectors(sh, pts, proj_l, tab, dr, "aos", misalign=mis)
+                        finally:
+                            sh.set_tuning("proj_aos_mode", 0)
+                            sh.set_tuning("proj_aos_split", 0)
+                            sh.set_tuning("proj_aos_pairs", 0)
+                        assert np.abs(got - want).max() <= TOL * max(1.0, np.abs(tab).max()), (n, mis, mode, split, pairs)
+                        if ref is None:
+                            ref = got
+                        assert np.array_equal(got, ref), (n, mis, mode, split, pairs)   # same arithmetic, different staging stores
 
 
 @pytest.mark.parametrize("form", [1, 2])
