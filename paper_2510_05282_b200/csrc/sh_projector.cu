@@ -358,8 +358,19 @@ template <int NV> struct ProjCfg;
 // compiler has 168 / 128 registers to overlap the polynomial chains of an l-block (a whole tile in ~7300 cycles, against 2 x 5700 for two
 // warps sharing it at 96 registers).  The ring holds 8 tiles at 100 columns, so 8 producers; the consumer warps follow from the FMA load:
 // four (G = 4: 32 accumulator registers) for up to four vectors, eight for eight.
-template <> struct ProjCfg<4> { static constexpr int NPW = 8, SPLIT = 1, NCW = 4, G = 4; };
-template <> struct ProjCfg<8> { static constexpr int NPW = 8, SPLIT = 1, NCW = 8, G = 4; };
+// Five to eight vectors: the contraction of a tile, coeff[8][ncols] += wts[8][32 points] x vals[ncols][32 points]^T, is a dense 8 x ncols x 32
+// product, and with DFMA consumers it was co-limited by shared-memory wavefronts (every lane re-reads its 8 weights per 4 values: ~1000
+// wavefronts per tile against 1490 cycles).  MMA = true hands it to the FP64 tensor-core instruction (mma.sync m8n8k4: A = weights of 4
+// points, B = values of 8 columns at those points): the same FP64 pipe time (on B200 DMMA runs at the DFMA rate and serialises with it), but
+// one A and <= 4 B fragment loads per 4 points and warp instead of 12 loads per point quarter, 2 accumulator doubles per 8 columns, and
+// 104 instead of 800 arithmetic issue slots per tile.  PITCH = 34 doubles between columns lets a fragment load (8 columns x 4 consecutive
+// points = 256 B) take the minimum of two wavefronts (column stride 272 B = 16 B mod 128: every bank is used exactly twice); with 32 the
+// eight columns fall on the same 32 bytes of banks.  The producers' stores (lane = point) are conflict-free for any pitch.  The wider
+// slots leave 7 in the ring at 100 columns, hence 7 producer warps.
+template <> struct ProjCfg<4> { static constexpr int NPW = 8, SPLIT = 1, NCW = 4, G = 4, PITCH = 32; static constexpr bool MMA = false; };
+// Measured on the 128^3 grid, 100 columns, 8 vectors (DFMA consumers, 8 + 8 warps: 0.354 ms): pitch 32 / 33 (8 slots, 8- / 4-way conflicts on the
+// fragment loads) 0.361 / 0.360; pitch 36, 8 producer warps of which 7 have a slot 0.277; pitch 34 (two wavefronts per load, as 36), 7 + 4 warps 0.272.
+template <> struct ProjCfg<8> { static constexpr int NPW = 7, SPLIT = 1, NCW = 4, G = 4, PITCH = 34; static constexpr bool MMA = true; };
 static_assert(ProjCfg<4>::SPLIT == ProjCfg<8>::SPLIT, "run_project builds one per-part channel list for both");
 
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
@@ -378,18 +389,66 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {   //
     } while (!done);
 }
 
+template <int PITCH>
 struct ProjectStage {
     double* sv;   // the tile slot's vals + lane
     const ProjPlan& plan;
     template <int L> __device__ __forceinline__ void block(const double (&blk)[2 * L + 1]) {
 #pragma unroll 1   // code size is instruction-fetch traffic (see ProjRowSink)
         for (int s = plan.first[L]; s < plan.first[L + 1]; ++s) {
-            double* q = sv + plan.col[s] * 32;
+            double* q = sv + plan.col[s] * PITCH;
             const double f = q[0];   // parked there by the radial pass
-            static_for<0, 2 * L + 1>([&](auto mc) { q[decltype(mc)::value * 32] = f * blk[decltype(mc)::value]; });
+            static_for<0, 2 * L + 1>([&](auto mc) { q[decltype(mc)::value * PITCH] = f * blk[decltype(mc)::value]; });
         }
     }
 };
+
+// The tensor-core consumer (ProjCfg::MMA): warp cw of NCW owns the 8-column tiles nt = cw + j * NCW, j < R (R = its count, warp-uniform:
+// the tile loop is compiled once per R and is branch-free inside).  Per 32-point tile and 4-point step ks: A fragment = wts[v = lane / 4]
+// [4 ks + lane % 4], B fragments = vals[8 nt + lane / 4][4 ks + lane % 4], D += A B (m8n8k4, fp64): D[v][8 nt + 2 (lane % 4) + {0, 1}] in this
+// lane.  The sums over the points are complete inside the instruction sequence, in a fixed order: no cross-lane reduction at the end.  A
+// column tile that reaches past ncols reads weight rows (inside the slot: ncols + 7 < ncols + NV) and its extra columns are not written out.
+template <int NV, int NCW, int PITCH, int R>
+__device__ __forceinline__ void project_consume_mma(const double* ring, int slot_doubles, int nring, uint64_t* full, uint64_t* empty, int64_t my_tiles,
+                                                    int ncols, int nvec, int cw, int lane, double* __restrict__ partial) {
+    static_assert(NV == 8, "m8n8k4: eight weight vectors are the M dimension");
+    const int grp = lane >> 2, tig = lane & 3;
+    double acc[R > 0 ? R : 1][2];
+    static_for<0, R>([&](auto jc) { acc[decltype(jc)::value][0] = 0.0; acc[decltype(jc)::value][1] = 0.0; });
+    int slot = 0, use = 0;
+    for (int64_t seq = 0; seq < my_tiles; ++seq) {
+        mbar_wait(full + slot, use & 1);
+        if constexpr (R > 0) {
+            const double* sv = ring + (size_t)slot * slot_doubles;
+            const double* arow = sv + (ncols + grp) * PITCH + tig;
+            const double* brow = sv + (8 * cw + grp) * PITCH + tig;
+#pragma unroll
+            for (int ks = 0; ks < 8; ++ks) {
+                const double a = arow[4 * ks];
+                double b[R];
+                static_for<0, R>([&](auto jc) { b[decltype(jc)::value] = brow[decltype(jc)::value * 8 * NCW * PITCH + 4 * ks]; });
+                static_for<0, R>([&](auto jc) {
+                    constexpr int J = decltype(jc)::value;
+                    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                                 : "+d"(acc[J][0]), "+d"(acc[J][1])
+                                 : "d"(a), "d"(b[J]));
+                });
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty + slot);
+        if (++slot == nring) { slot = 0; ++use; }
+    }
+    static_for<0, R>([&](auto jc) {
+        constexpr int J = decltype(jc)::value;
+        const int c = 8 * (cw + J * NCW) + 2 * tig;
+        if (grp < nvec) {
+            double* row = partial + ((int64_t)blockIdx.x * nvec + grp) * ncols;
+            if (c < ncols) row[c] = acc[J][0];
+            if (c + 1 < ncols) row[c + 1] = acc[J][1];
+        }
+    });
+}
 
 // The consumer side of sh_project_kernel for a warp whose lanes own R columns each (column owner + j * OWNERS, j < R).
 template <int NV, int G, int OWNERS, int R>
@@ -443,12 +502,12 @@ __global__ void __launch_bounds__(32 * (ProjCfg<NV>::NPW + ProjCfg<NV>::NCW), 1)
     sh_project_kernel(const double* __restrict__ xyz, int64_t n, const double* __restrict__ radial, const __grid_constant__ ProjPlan plan,
                       const double* __restrict__ w, int nvec, double* __restrict__ partial, int nring) {
     using Cfg = ProjCfg<NV>;
-    constexpr int NPW = Cfg::NPW, SPLIT = Cfg::SPLIT, NCW = Cfg::NCW, G = Cfg::G;
-    static_assert(NPW % SPLIT == 0 && 32 % G == 0 && NV >= G - 1, "shape");
+    constexpr int NPW = Cfg::NPW, SPLIT = Cfg::SPLIT, NCW = Cfg::NCW, G = Cfg::G, PITCH = Cfg::PITCH;
+    static_assert(NPW % SPLIT == 0 && 32 % G == 0 && NV >= G - 1 && PITCH >= 32, "shape");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int ncols = plan.ncols;
-    const int slot_doubles = (ncols + NV) * 32;
+    const int slot_doubles = (ncols + NV) * PITCH;
     double* ring = reinterpret_cast<double*>(smem_raw);
     uint64_t* full = reinterpret_cast<uint64_t*>(ring + (size_t)nring * slot_doubles);
     uint64_t* empty = full + PROJ_RING_MAX;
@@ -464,8 +523,13 @@ __global__ void __launch_bounds__(32 * (ProjCfg<NV>::NPW + ProjCfg<NV>::NCW), 1)
 
     if (warp < NPW) {
         // ---------------- producer ----------------
-        constexpr int STREAMS = NPW / SPLIT;
+        // Tile streams: at most as many as the ring has slots.  With more streams than slots a producer could be TWO uses ahead of a slot,
+        // and a parity wait cannot tell "the use before last is still being read" from "the last use has been released" (DESIGN.md
+        // section 6: it hangs, after racing); with streams <= slots the stream's own previous tile guarantees the older release.
+        constexpr int MAX_STREAMS = NPW / SPLIT;
+        const int STREAMS = MAX_STREAMS < nring ? MAX_STREAMS : nring;
         const int stream = warp / SPLIT, part = warp % SPLIT;
+        if (stream >= STREAMS) return;   // a producer warp without a stream (only when the ring is shorter than the warp list)
         const int ps0 = plan.part_first[part], ps1 = plan.part_first[part + 1];   // this warp's channel slots
         // point index of this lane in the stream's current tile; the stream advances by STREAMS * gridDim.x tiles
         int64_t i = (((int64_t)blockIdx.x + (int64_t)stream * gridDim.x) << 5) + lane;
@@ -500,17 +564,17 @@ __global__ void __launch_bounds__(32 * (ProjCfg<NV>::NPW + ProjCfg<NV>::NCW), 1)
 #pragma unroll 8   // eight channels' table loads in flight (4: 0.230 ms, 8: 0.228, 16: 0.279 for four vectors on the 128^3 grid)
             for (int k = ps0; k < ps1; ++k) {
                 const int s = plan.part_slots[k];
-                sv[plan.col[s] * 32] = pos.f_row(radial + plan.row[s]);
+                sv[plan.col[s] * PITCH] = pos.f_row(radial + plan.row[s]);
             }
             const UnitVec u = normalize(x, y, z);
-            ProjectStage sink{sv, plan};
+            ProjectStage<PITCH> sink{sv, plan};
             static_for<0, SPLIT>([&](auto pc) {
                 constexpr int PART = decltype(pc)::value;
                 if (part == PART) eval_projector_blocks<LMAX, FAST, SPLIT, PART>(u, plan, sink);
             });
             static_for<0, WPP>([&](auto kc) {
                 const int v = part + decltype(kc)::value * SPLIT;
-                if (v < NV) sv[(ncols + v) * 32] = (ok && v < nvec) ? wv[decltype(kc)::value] : 0.0;
+                if (v < NV) sv[(ncols + v) * PITCH] = (ok && v < nvec) ? wv[decltype(kc)::value] : 0.0;
             });
             __syncwarp();
             if (lane == 0) mbar_arrive(full + slot);
@@ -520,15 +584,26 @@ __global__ void __launch_bounds__(32 * (ProjCfg<NV>::NPW + ProjCfg<NV>::NCW), 1)
         }
     } else {
         // ---------------- consumer ----------------
-        constexpr int OWNERS = NCW * G, CPW = (PROJ_MAX_COLS + OWNERS - 1) / OWNERS;
         const int cw = warp - NPW;
-        // column rounds of the warp's first owner (warp-uniform): the tile loop is compiled once per count, branch-free inside
-        const int rounds = (ncols - cw * G + OWNERS - 1) / OWNERS;
-        static_for<0, CPW + 1>([&](auto rc) {
-            constexpr int R = decltype(rc)::value;
-            if ((rounds < 0 ? 0 : rounds) == R)
-                project_consume<NV, G, OWNERS, R>(ring, slot_doubles, nring, full, empty, my_tiles, ncols, nvec, cw, lane, partial);
-        });
+        if constexpr (Cfg::MMA) {
+            constexpr int RMAX = ((PROJ_MAX_COLS + 7) / 8 + NCW - 1) / NCW;   // 8-column tiles per warp
+            const int ntiles8 = (ncols + 7) >> 3;
+            const int mine = ntiles8 > cw ? (ntiles8 - cw + NCW - 1) / NCW : 0;   // warp-uniform
+            static_for<0, RMAX + 1>([&](auto rc) {
+                constexpr int R = decltype(rc)::value;
+                if (mine == R) project_consume_mma<NV, NCW, PITCH, R>(ring, slot_doubles, nring, full, empty, my_tiles, ncols, nvec, cw, lane, partial);
+            });
+        } else {
+            static_assert(PITCH == 32, "project_consume reads rows of 32 doubles");
+            constexpr int OWNERS = NCW * G, CPW = (PROJ_MAX_COLS + OWNERS - 1) / OWNERS;
+            // column rounds of the warp's first owner (warp-uniform): the tile loop is compiled once per count, branch-free inside
+            const int rounds = (ncols - cw * G + OWNERS - 1) / OWNERS;
+            static_for<0, CPW + 1>([&](auto rc) {
+                constexpr int R = decltype(rc)::value;
+                if ((rounds < 0 ? 0 : rounds) == R)
+                    project_consume<NV, G, OWNERS, R>(ring, slot_doubles, nring, full, empty, my_tiles, ncols, nvec, cw, lane, partial);
+            });
+        }
     }
 }
 
@@ -759,7 +834,7 @@ int launch_project_ring(const double* xyz, int64_t n, const double* radial, cons
                         int64_t* rows, cudaStream_t st) {
     using Cfg = ProjCfg<NV>;
     // ring of tile slots: as many as fit (at most PROJ_RING_MAX), then the 2 x PROJ_RING_MAX mbarriers
-    const size_t slot_bytes = (size_t)(plan.ncols + NV) * 32 * sizeof(double);
+    const size_t slot_bytes = (size_t)(plan.ncols + NV) * Cfg::PITCH * sizeof(double);
     int nring = (int)(((size_t)227 * 1024 - 2 * PROJ_RING_MAX * sizeof(uint64_t)) / slot_bytes);
     if (nring > PROJ_RING_MAX) nring = PROJ_RING_MAX;
     if (nring < 1) return SH_ERR_PROJECTOR;
