@@ -363,14 +363,16 @@ template <int NV> struct ProjCfg;
 // wavefronts per tile against 1490 cycles).  MMA = true hands it to the FP64 tensor-core instruction (mma.sync m8n8k4: A = weights of 4
 // points, B = values of 8 columns at those points): the same FP64 pipe time (on B200 DMMA runs at the DFMA rate and serialises with it), but
 // one A and <= 4 B fragment loads per 4 points and warp instead of 12 loads per point quarter, 2 accumulator doubles per 8 columns, and
-// 104 instead of 800 arithmetic issue slots per tile.  PITCH = 34 doubles between columns lets a fragment load (8 columns x 4 consecutive
-// points = 256 B) take the minimum of two wavefronts (column stride 272 B = 16 B mod 128: every bank is used exactly twice); with 32 the
-// eight columns fall on the same 32 bytes of banks.  The producers' stores (lane = point) are conflict-free for any pitch.  The wider
-// slots leave 7 in the ring at 100 columns, hence 7 producer warps.
+// 104 instead of 800 arithmetic issue slots per tile.  What it needs is conflict-free FRAGMENT loads: a fragment is 8 columns x 4
+// consecutive points, and 64-bit shared loads are served per half-warp, so the four columns of a half-warp must tile 128 bytes: a column
+// pitch of 36 doubles (288 B = 32 B mod 128).  With 32 the eight columns fall on the same 32 bytes of banks (no gain at all), 34 still leaves
+// 2-way conflicts (ncu: 3.9 wavefronts per load).  The producers' stores (lane = point) are conflict-free for any pitch.  The wider slots
+// leave 7 in the ring at 100 columns, hence 7 producer warps.
 template <> struct ProjCfg<4> { static constexpr int NPW = 8, SPLIT = 1, NCW = 4, G = 4, PITCH = 32; static constexpr bool MMA = false; };
-// Measured on the 128^3 grid, 100 columns, 8 vectors (DFMA consumers, 8 + 8 warps: 0.354 ms): pitch 32 / 33 (8 slots, 8- / 4-way conflicts on the
-// fragment loads) 0.361 / 0.360; pitch 36, 8 producer warps of which 7 have a slot 0.277; pitch 34 (two wavefronts per load, as 36), 7 + 4 warps 0.272.
-template <> struct ProjCfg<8> { static constexpr int NPW = 7, SPLIT = 1, NCW = 4, G = 4, PITCH = 34; static constexpr bool MMA = true; };
+// Measured on the 128^3 grid, 100 columns, 8 vectors (DFMA consumers, 8 + 8 warps: 0.354 ms): pitch 32 / 33 (8 slots, conflicting fragment loads)
+// 0.361 / 0.360; pitch 34, 7 + 4 warps 0.272; pitch 36, 7 + 4 warps 0.265; pitch 32 with the point index of a column XOR-swizzled by its position
+// in its channel (conflict-free at 8 slots and 8 producers, a per-column table for the consumers) 0.267 -- no better, so the plain pitch stays.
+template <> struct ProjCfg<8> { static constexpr int NPW = 7, SPLIT = 1, NCW = 4, G = 4, PITCH = 36; static constexpr bool MMA = true; };
 static_assert(ProjCfg<4>::SPLIT == ProjCfg<8>::SPLIT, "run_project builds one per-part channel list for both");
 
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
