@@ -105,6 +105,23 @@ __device__ __forceinline__ UnitVec normalize(double x, double y, double z) {
     return u;
 }
 
+// a2 for the fp32 variant (fp32 coordinates in, unit vector rounded once to fp32).  The fp64 range scaling is not needed (the square of
+// any fp32 value, subnormals included, is a normal fp64 number), and 1/sqrt comes from the fp64 rsqrt (reciprocal-square-root seed + Newton
+// steps, <= 2 ulp in fp64: nine orders below the rounding to fp32 that follows) instead of an IEEE sqrt and an IEEE divide, which together
+// are ~150 instructions -- a third of this variant's instruction stream when two warps share a point group.  Results are defined by
+// SURVEY.md 8c #21 ("normalization in fp64, rounded once to fp32") and by the 1e-5 tolerance; r = 0, NaN and Inf as in normalize().
+__device__ __forceinline__ UnitVec normalize_f32in(float xf, float yf, float zf) {
+    const double x = xf, y = yf, z = zf;
+    const double r2 = x * x + y * y + z * z;
+    UnitVec u;
+    u.origin = (r2 == 0.0);
+    double inv = rsqrt(r2);
+    if (u.origin) inv = 0.0;
+    if (!(r2 <= DBL_MAX)) inv = __longlong_as_double(0x7ff8000000000000LL);
+    u.x = x * inv; u.y = y * inv; u.z = z * inv;
+    return u;
+}
+
 // Normalized-Cartesian front end (the paper's fastest interface): the caller guarantees x^2+y^2+z^2 = 1
 // (Eq. 8); a2 is skipped.  A zero vector selects the r = 0 convention.
 __device__ __forceinline__ UnitVec as_given(double x, double y, double z) {
@@ -145,7 +162,8 @@ struct RawPoint {
     __device__ __forceinline__ UnitVec unit(int coords) const {
         if constexpr (ANGULAR) return from_angles((double)x, (double)y);
         if (coords == SH_COORDS_NORMALIZED) return as_given((double)x, (double)y, (double)z);
-        return normalize((double)x, (double)y, (double)z);
+        if constexpr (std::is_same<TI, float>::value) return normalize_f32in(x, y, z);
+        else return normalize((double)x, (double)y, (double)z);
     }
 };
 

@@ -142,7 +142,7 @@ __global__ void __launch_bounds__(256) sh_soa_pair_kernel(const float* __restric
     SoAPairSink sink{out + 2 * j, n};
     // one copy of the polynomial code: only the front end branches (straight-line code size is instruction-fetch traffic)
     UnitVec u0, u1;
-    if (coords == SH_COORDS_CARTESIAN) { u0 = normalize(ca.x, ca.y, cb.x); u1 = normalize(cb.y, cc.x, cc.y); }
+    if (coords == SH_COORDS_CARTESIAN) { u0 = normalize_f32in(ca.x, ca.y, cb.x); u1 = normalize_f32in(cb.y, cc.x, cc.y); }
     else { u0 = as_given(ca.x, ca.y, cb.x); u1 = as_given(cb.y, cc.x, cc.y); }
     evaluate_pair<LMAX>(u0, u1, sink);
 }
