@@ -116,6 +116,26 @@ def test_every_lmax_unsorted_channels_and_ragged_sizes(sh, oracle_mod, lmax):
             check_project(gpu_project(sh, pts, proj_l, tab, dr, w), coeff, abs_sum)
 
 
+@pytest.mark.parametrize("proj_l", [[0], [1], [0, 1, 1], [2, 1], [4], [3, 3, 0], [7], [9, 9, 9, 9, 9, 4]])
+def test_project_five_to_eight_vectors_column_tile_edges(sh, oracle_mod, proj_l):
+    """5 to 8 weight vectors contract on the FP64 tensor-core instruction in tiles of 8 columns x 4 points: column counts of 1, 3, 7, 8, 9,
+    15, 15 and 104 (one column, just below / at / just above a tile, the widest single pass), fewer vectors than the 8 rows of the instruction,
+    one point, a ragged last 32-point tile, and enough tiles for every CTA of the persistent grid to wrap around its ring of slots."""
+    rng = np.random.default_rng(900 + len(proj_l) * 17 + proj_l[0])
+    nr, dr = 41, 0.08
+    tab = rng.standard_normal((len(proj_l), nr))
+    tab[:, -1] = 0.0
+    for n in (1, 33, 4097, 148 * 32 * 9 + 5):
+        g = rng.standard_normal((n, 3))
+        pts = g / np.linalg.norm(g, axis=1)[:, None] * rng.uniform(0.0, 3.4, n)[:, None]
+        for nvec in (5, 8):
+            w = rng.standard_normal((nvec, n))
+            coeff, abs_sum = oracle_mod.project(pts, proj_l, tab, dr, w)
+            got = gpu_project(sh, pts, proj_l, tab, dr, w)
+            check_project(got, coeff, abs_sum)
+            assert np.array_equal(got, gpu_project(sh, pts, proj_l, tab, dr, w)), (n, nvec)   # fixed summation order
+
+
 @pytest.mark.parametrize("proj_l", [[2], [0, 1, 3], [1, 1], [0, 2, 1, 3], [9, 9, 9, 4, 0], [0, 1, 2, 3, 4, 5, 6, 7, 8, 9], [5, 4, 4, 7], [9] * 11, [9] * 12])
 def test_aos_store_modes(sh, oracle_mod, proj_l):
     """AoS copy-out modes of sh_projectors: odd ncols (one bulk copy per tile), even ncols with ncols/2 odd or even (one
