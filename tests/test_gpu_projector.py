@@ -200,7 +200,7 @@ def test_project_polynomial_forms_value_by_value(sh, oracle_mod, form):
     assert err <= TOL * max(1.0, np.abs(tab).max())
 
 
-@pytest.mark.parametrize("nvec", [1, 4])
+@pytest.mark.parametrize("nvec", [1, 4, 8])
 def test_project_factorized_forms_full_grid(sh, oracle_mod, nvec):
     """The factorized forms (knob value 2; the default is Horner / recurrence) on the bench's FP64-bound workload (128^3 grid,
     100 columns) against the oracle's sum."""
@@ -299,11 +299,13 @@ def test_full_grid_moments_lmax9(sh, oracle_mod):
 
     pts = inputs.config3_full_grid()
     proj_l, tab, dr = inputs.projector_channels(lmax=9, per_l=1, cutoff=6.0, dr=0.02)
-    w = inputs.wave_weights(len(pts), 2, seed=8, volume_element=(12.0 / 128) ** 3)
-    got = gpu_project(sh, pts, proj_l, tab, dr, w)
+    w = inputs.wave_weights(len(pts), 8, seed=8, volume_element=(12.0 / 128) ** 3)
     coeff, abs_sum = oracle_mod.project(pts, proj_l, tab, dr, w)
-    worst = check_project(got, coeff, abs_sum)
-    print(f"full grid projection: max |c_gpu - c_oracle| / sum|terms| = {worst:.2e}")
+    # one vector: segment kernel; two and four: ring kernel with DFMA consumers; eight: ring kernel contracting on the FP64 tensor-core instruction
+    for nvec in (1, 2, 4, 8):
+        got = gpu_project(sh, pts, proj_l, tab, dr, w[:nvec])
+        worst = check_project(got, coeff[:nvec], abs_sum[:nvec])
+        print(f"full grid projection, {nvec} vectors: max |c_gpu - c_oracle| / sum|terms| = {worst:.2e}")
     import torch
 
     x = torch.from_numpy(pts).cuda()
